@@ -1,0 +1,169 @@
+"""ctypes wrapper of the CPU oracle oracle/liborc.so (TEST INFRASTRUCTURE, not the product).
+
+Argument marshalling only; every formula lives in oracle/orc.c, which cites the
+passages of PAPER.md / DESIGN.md it follows.  Arrays are C-contiguous float64 numpy
+arrays in the layout U[b][c][k][j][i] (ghosted) and A[b][c][k][j][i] (interior).
+"""
+import ctypes as C
+
+import numpy as np
+
+from . import build as _build
+
+
+class OrcParams(C.Structure):
+    _fields_ = [("nx", C.c_int), ("ny", C.c_int), ("nz", C.c_int), ("ng", C.c_int),
+                ("nbx", C.c_int), ("nby", C.c_int), ("nbz", C.c_int), ("nspec", C.c_int),
+                ("dx", C.c_double), ("dy", C.c_double), ("dz", C.c_double),
+                ("gamma", C.c_double), ("grav", C.c_double * 3),
+                ("bc_lo", C.c_int * 3), ("bc_hi", C.c_int * 3),
+                ("small_dens", C.c_double), ("small_pres", C.c_double)]
+
+
+_lib = None
+_dp = C.POINTER(C.c_double)
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        _lib = C.CDLL(_build.build())
+        P = C.POINTER(OrcParams)
+        _lib.orc_fill_ghosts.argtypes = [P, _dp]
+        _lib.orc_advance_A.argtypes = [P, _dp, _dp]
+        _lib.orc_sdc_update.argtypes = [P, _dp, _dp, C.c_double, _dp, _dp, C.c_int,
+                                        C.POINTER(_dp), _dp]
+        _lib.orc_cfl_dt.argtypes = [P, _dp, C.c_double, _dp]
+        _lib.orc_cons_to_prim.argtypes = [C.c_int, C.c_double, C.c_double, _dp, _dp]
+        _lib.orc_cons_to_prim.restype = None
+        _lib.orc_ppm_line.argtypes = [C.c_int, _dp, _dp, _dp]
+        _lib.orc_ppm_line.restype = None
+        _lib.orc_hllc.argtypes = [C.c_int, C.c_int, C.c_double, _dp, _dp, _dp]
+        _lib.orc_hllc.restype = None
+        _lib.orc_exact_riemann_star.argtypes = [C.c_double] * 7 + [_dp]
+        _lib.orc_exact_riemann_sample.argtypes = [C.c_double] * 7 + [C.c_int, _dp, _dp, _dp, _dp]
+        _lib.orc_num_threads.restype = C.c_int
+    return _lib
+
+
+def make_params(cfg: dict) -> OrcParams:
+    """cfg: the plain dict produced by paper_1910_12578_b200.workloads (keys = field names)."""
+    p = OrcParams()
+    for k in ("nx", "ny", "nz", "ng", "nbx", "nby", "nbz", "nspec"):
+        setattr(p, k, int(cfg[k]))
+    for k in ("dx", "dy", "dz", "gamma", "small_dens", "small_pres"):
+        setattr(p, k, float(cfg[k]))
+    for d in range(3):
+        p.grav[d] = float(cfg["grav"][d])
+        p.bc_lo[d] = int(cfg["bc_lo"][d])
+        p.bc_hi[d] = int(cfg["bc_hi"][d])
+    return p
+
+
+def _ptr(a):
+    assert a.dtype == np.float64 and a.flags["C_CONTIGUOUS"]
+    return a.ctypes.data_as(_dp)
+
+
+def _chk(rc, what):
+    if rc != 0:
+        raise RuntimeError(f"oracle {what} failed with code {rc}")
+
+
+def u_shape(cfg):
+    ng = cfg["ng"]
+    return (cfg["nbx"] * cfg["nby"] * cfg["nbz"], 5 + cfg["nspec"],
+            cfg["nz"] + 2 * ng, cfg["ny"] + 2 * ng, cfg["nx"] + 2 * ng)
+
+
+def a_shape(cfg):
+    return (cfg["nbx"] * cfg["nby"] * cfg["nbz"], 5 + cfg["nspec"], cfg["nz"], cfg["ny"], cfg["nx"])
+
+
+def fill_ghosts(cfg, U):
+    assert U.shape == u_shape(cfg)
+    _chk(lib().orc_fill_ghosts(C.byref(make_params(cfg)), _ptr(U)), "fill_ghosts")
+    return U
+
+
+def advance_A(cfg, U, A=None):
+    assert U.shape == u_shape(cfg)
+    if A is None:
+        A = np.empty(a_shape(cfg), dtype=np.float64)
+    _chk(lib().orc_advance_A(C.byref(make_params(cfg)), _ptr(U), _ptr(A)), "advance_A")
+    return A
+
+
+def sdc_update(cfg, U_next, U_m, dt_m, A_new_m, A_old_m, A_quad, w_quad):
+    n = len(A_quad)
+    arr = (_dp * max(n, 1))(*[_ptr(a) for a in A_quad])
+    w = np.ascontiguousarray(np.asarray(w_quad, dtype=np.float64))
+    _chk(lib().orc_sdc_update(C.byref(make_params(cfg)), _ptr(U_next), _ptr(U_m), float(dt_m),
+                              _ptr(A_new_m), _ptr(A_old_m), n, arr, _ptr(w) if n else None),
+         "sdc_update")
+    return U_next
+
+
+def cfl_dt(cfg, U, cfl):
+    out = C.c_double(0.0)
+    _chk(lib().orc_cfl_dt(C.byref(make_params(cfg)), _ptr(U), float(cfl), C.byref(out)), "cfl_dt")
+    return out.value
+
+
+def cons_to_prim(gamma, small_pres, Uz):
+    Uz = np.ascontiguousarray(Uz, dtype=np.float64)
+    Wz = np.empty_like(Uz)
+    lib().orc_cons_to_prim(len(Uz), gamma, small_pres, _ptr(Uz), _ptr(Wz))
+    return Wz
+
+
+def ppm_line(q):
+    """Returns (qm, qp); valid for zones 2..n-3, NaN elsewhere."""
+    q = np.ascontiguousarray(q, dtype=np.float64)
+    qm = np.full_like(q, np.nan)
+    qp = np.full_like(q, np.nan)
+    lib().orc_ppm_line(len(q), _ptr(q), _ptr(qm), _ptr(qp))
+    return qm, qp
+
+
+def hllc(d, gamma, WL, WR):
+    WL = np.ascontiguousarray(WL, dtype=np.float64)
+    WR = np.ascontiguousarray(WR, dtype=np.float64)
+    F = np.empty_like(WL)
+    lib().orc_hllc(len(WL), d, gamma, _ptr(WL), _ptr(WR), _ptr(F))
+    return F
+
+
+def exact_riemann_star(g, rL, uL, pL, rR, uR, pR):
+    out = np.zeros(5)
+    lib().orc_exact_riemann_star(g, rL, uL, pL, rR, uR, pR, _ptr(out))
+    return out
+
+
+def exact_riemann_sample(g, rL, uL, pL, rR, uR, pR, xi):
+    xi = np.ascontiguousarray(xi, dtype=np.float64).ravel()
+    rho, u, p = np.empty_like(xi), np.empty_like(xi), np.empty_like(xi)
+    lib().orc_exact_riemann_sample(g, rL, uL, pL, rR, uR, pR, len(xi), _ptr(xi), _ptr(rho), _ptr(u), _ptr(p))
+    return rho, u, p
+
+
+def num_threads():
+    return lib().orc_num_threads()
+
+
+# ---- harness-level SDC driver (SURVEY 8(c) S5 "Driver") ------------------------
+def sdc_step_2nd(cfg, U, dt):
+    """One 2-node, 2-iteration SDC step (trapezoid) with R = 0, built only from
+    oracle calls: ghost fill, A, node update.  U: ghosted state with interior valid; returns new U."""
+    U0 = fill_ghosts(cfg, U.copy())
+    A0 = advance_A(cfg, U0)
+    w = [0.5 * dt, 0.5 * dt]
+    # iteration 1: all nodes carry A(U^n)
+    U1 = U0.copy()
+    sdc_update(cfg, U1, U0, dt, A0, A0, [A0, A0], w)
+    fill_ghosts(cfg, U1)
+    A1 = advance_A(cfg, U1)
+    # iteration 2: node 0 unchanged => A-difference term is zero; integral uses iteration-1 values
+    U2 = U0.copy()
+    sdc_update(cfg, U2, U0, dt, A0, A0, [A0, A1], w)
+    return U2
