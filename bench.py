@@ -1,0 +1,352 @@
+#!/usr/bin/env python
+"""bench.py -- zone-updates/s of the fp64 A(U)+SDC hot path on B200 (BASELINE.json metric).
+
+One "step" = one pass of the whole hot path over the workload:
+    cst_fill_ghosts(U) -> cst_advance_A_update(U -> A_new, U_next) -> cst_cfl_dt_device(U)
+with the state not evolving between steps (outputs go to second buffers), inputs resident in HBM.
+Default workload: BASELINE.json configs[3] (512^3 periodic box, NVAR = 18); --workload 4 runs the
+XRB-shaped batch of 512 boxes of 64^3.  Prints ONE JSON line (rank 0).
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload 3|4] [--impl ours|reference]
+Multi-GPU: launched by torchrun, one rank per GPU; every rank runs the workload on its own
+replica of the domain (weak scaling, no data-path collective; dt is all-reduced with MIN).
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+from concurrent.futures import ThreadPoolExecutor
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+from paper_1910_12578_b200 import workloads as wl  # noqa: E402
+
+METRIC = "zone-updates/s of fp64 A(U)+SDC update"
+UNIT = "zone-updates/s"
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", type=int, default=3, choices=[0, 1, 2, 3, 4])
+    ap.add_argument("--n", type=int, default=None, help="override zones per box side (debug only; marks the line)")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    return ap.parse_args()
+
+
+# ------------------------------------------------------------------------------------ bytes ----
+def alg_bytes(cfg):
+    """Algorithmic bytes per zone-update, strict count."""
+    ng, nx, ny, nz, N = cfg["ng"], cfg["nx"], cfg["ny"], cfg["nz"], wl.nvar(cfg)
+    G = (nx + 2 * ng) * (ny + 2 * ng) * (nz + 2 * ng) / (nx * ny * nz)
+    G3 = 1.0 + 6.0 * (1.0 / nx + 1.0 / ny + 1.0 / nz)
+    fill = 2.0 * (G - 1.0) * N * 8.0                 # read source + write ghost, full shell
+    adv = (G3 + 4.0) * N * 8.0                       # U (+3-deep face ghosts), A_old^m, A_old^other, A_new, U_next
+    cfl = 5.0 * 8.0                                  # hydro components of the interior
+    return dict(fill=fill, advance=adv, cfl=cfl, step=fill + adv + cfl, G=G, G3=G3)
+
+
+def measured_peaks():
+    try:
+        mp = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+        return float(mp["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+# ----------------------------------------------------------------------------------- inputs ----
+def fill_host_state(cfg, U_host_np, threads=8):
+    """Seeded synthetic state of the config, plane by plane, into the host array (ghosts zero)."""
+    Dz = wl.domain(cfg)[2]
+
+    def one(kg):
+        wl.scatter_plane(cfg, U_host_np, kg, wl.cons_plane(cfg, kg))
+    with ThreadPoolExecutor(threads) as ex:
+        list(ex.map(one, range(Dz)))
+
+
+def host_mem_available():
+    """Bytes of host memory this process may still take (MemAvailable, capped by the cgroup limit)."""
+    avail = 1 << 62
+    try:
+        for line in open("/proc/meminfo"):
+            if line.startswith("MemAvailable"):
+                avail = int(line.split()[1]) * 1024
+    except Exception:
+        pass
+    try:
+        lim = open("/sys/fs/cgroup/memory.max").read().strip()
+        cur = int(open("/sys/fs/cgroup/memory.current").read().strip())
+        if lim != "max":
+            avail = min(avail, int(lim) - cur)
+    except Exception:
+        pass
+    return avail
+
+
+# ----------------------------------------------------------------------------------- clocks ----
+class ClockSampler:
+    FIELDS = ["clocks.sm", "clocks.max.sm", "power.draw", "clocks_event_reasons.hw_slowdown",
+              "clocks_event_reasons.hw_thermal_slowdown", "clocks_event_reasons.sw_thermal_slowdown",
+              "clocks_event_reasons.sw_power_cap"]
+
+    def __init__(self, index):
+        self.rows, self.proc = [], None
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(index), "--query-gpu=" + ",".join(self.FIELDS),
+                 "--format=csv,noheader,nounits", "-lms", "100"],
+                stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append((time.time(), [x.strip() for x in line.split(",")]))
+
+    def stop(self, t0, t1):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        rows = [r for (t, r) in self.rows if t0 <= t <= t1 + 0.1] or [r for (_, r) in self.rows]
+        sm, mx, reasons = [], [], set()
+        for r in rows:
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1]))
+            except Exception:
+                continue
+            for name, v in zip(["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"], r[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+# ------------------------------------------------------------------------------ CPU baseline ----
+def oracle_sample_cfg(cfg):
+    """A bounded sample of the same workload for the CPU oracle (~10-30 s of CPU work)."""
+    if cfg["index"] == 4:
+        c = wl.make_config(4, n=(cfg["nx"], cfg["ny"], cfg["nz"]), nb=(2, 2, cfg["nbz"]), nspec=cfg["nspec"])
+        what = f"{c['nbx'] * c['nby'] * c['nbz']} of the {cfg['nbx'] * cfg['nby'] * cfg['nbz']} boxes (2x2 columns, full height)"
+    else:
+        n = min(cfg["nx"], 144)
+        c = wl.make_config(cfg["index"], n=n, nspec=cfg["nspec"])
+        what = f"same input distribution on a {n}^3 box (1 of {max(1, (cfg['nx'] // n) ** 3)} sub-volumes)"
+    return c, what
+
+
+def time_oracle(cfg, steps, warmup):
+    from oracle import orc   # the one other place the oracle may run: the timed CPU baseline
+    c, what = oracle_sample_cfg(cfg)
+    U = wl.initial_state(c, ghost_value=0.0)
+    Un = U.copy()
+    A_old0, A_old1 = np.zeros(wl.a_shape(c)), np.zeros(wl.a_shape(c))
+    times = []
+    for s in range(warmup + steps):
+        t0 = time.perf_counter()
+        orc.fill_ghosts(c, U)
+        dt = orc.cfl_dt(c, U, 0.5)
+        A = orc.advance_A(c, U)
+        orc.sdc_update(c, Un, U, dt, A, A_old0, [A_old0, A_old1], [0.5 * dt, 0.5 * dt])
+        if s >= warmup:
+            times.append(time.perf_counter() - t0)
+    zones = wl.nzones(c)
+    return dict(value=zones / float(np.mean(times)), unit=UNIT, cores=orc.num_threads(), kind="oracle",
+                sample=what + f"; {steps} timed passes of fill_ghosts+cfl+A+update, {zones} zones each"), float(np.mean(times))
+
+
+def run_reference(args, cfg, rank):
+    if rank != 0:
+        return
+    steps, warmup = max(1, min(args.steps, 3)), max(0, min(args.warmup, 1))
+    cb, sec = time_oracle(cfg, steps, warmup)
+    line = {"impl": "reference", "metric": METRIC, "value": cb["value"], "unit": UNIT, "n_gpus": args.gpus,
+            "steps": steps, "warmup": warmup, "ms_per_step": sec * 1e3, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": f"configs[{cfg['index']}] {cfg['name']} (bounded sample: {cb['sample']})"},
+            "cpu_baseline": cb,
+            "e2e": {"value": cb["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line), flush=True)
+
+
+# -------------------------------------------------------------------------------------- main ----
+def main():
+    args = parse()
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    cfg = wl.make_config(args.workload, n=args.n) if args.n else wl.make_config(args.workload)
+
+    if args.impl == "reference":
+        run_reference(args, cfg, rank)
+        return
+
+    import torch
+    import torch.distributed as dist
+    from paper_1910_12578_b200 import Context
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (no CPU fallback)")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+
+    ctx = Context(cfg)
+    N, zones = wl.nvar(cfg), wl.nzones(cfg)
+    ushape, ashape = wl.u_shape(cfg), wl.a_shape(cfg)
+    ubytes, abytes = int(np.prod(ushape)) * 8, int(np.prod(ashape)) * 8
+
+    # ---- host input (pinned if possible), seeded + synthetic --------------------------------
+    pinned = True
+    try:
+        U_host = torch.zeros(ushape, dtype=torch.float64, pin_memory=True)
+    except Exception:
+        pinned = False
+        U_host = torch.zeros(ushape, dtype=torch.float64)
+    fill_host_state(cfg, U_host.numpy())
+
+    U = torch.empty(ushape, dtype=torch.float64, device=dev)
+    U.copy_(U_host, non_blocking=True)
+    U_next = U.clone()
+    A_new = torch.empty(ashape, dtype=torch.float64, device=dev)
+    A_old0 = torch.zeros(ashape, dtype=torch.float64, device=dev)
+    A_old1 = torch.zeros(ashape, dtype=torch.float64, device=dev)
+    dt_dev = torch.zeros(1, dtype=torch.float64, device=dev)
+    ctx.fill_ghosts(U)
+    dt = ctx.cfl_dt(U, 0.5)
+    if world > 1:
+        t = torch.tensor([dt], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MIN)
+        dt = float(t.item())
+    # A_old buffers hold plausible values: A of the initial state and a perturbation of it
+    ctx.advance_A(U, A_old0)
+    A_old1.copy_(A_old0).mul_(0.9)
+    w = [0.5 * dt, 0.5 * dt]
+
+    ev = lambda: torch.cuda.Event(enable_timing=True)
+    k_ev = []
+
+    def step(timed):
+        ctx.fill_ghosts(U)
+        if timed:
+            e0, e1 = ev(), ev()
+            e0.record()
+        ctx.advance_A_update(U, A_new, U_next, dt, A_old0, [A_old0, A_old1], w)
+        if timed:
+            e1.record()
+            k_ev.append((e0, e1))
+        ctx.cfl_dt_device(U, 0.5, dt_dev)
+
+    def sync_all():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        step(False)
+    sync_all()
+    sampler = ClockSampler(local) if rank == 0 else None
+    l0 = ctx.launch_count()
+    t_wall0 = time.time()
+    s0, s1 = ev(), ev()
+    s0.record()
+    for _ in range(args.steps):
+        step(True)
+    s1.record()
+    sync_all()
+    t_wall1 = time.time()
+    launches = ctx.launch_count() - l0
+    ms = s0.elapsed_time(s1)
+    if world > 1:
+        t = torch.tensor([ms], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    clocks = sampler.stop(t_wall0, t_wall1) if sampler else None
+    ms_step = ms / args.steps
+    value = zones * world / (ms_step * 1e-3)
+    k_ms = float(np.mean([a.elapsed_time(b) for a, b in k_ev]))
+
+    # ---- roofline of the dominant kernel (the fused advance+update kernel) ------------------
+    ab = alg_bytes(cfg)
+    peak, peak_src = measured_peaks()
+    achieved = ab["advance"] * zones / (k_ms * 1e-3) / 1e9
+    traffic = None
+    try:
+        tj = json.load(open(os.path.join(ROOT, "profiles", "traffic.json")))
+        traffic = tj.get(f"configs[{cfg['index']}]", {}).get("advance_dram_bytes_per_launch")
+    except Exception:
+        pass
+    roofline = {"bound": "hbm", "kernel": "advance_A_update (S1-S5)", "achieved": achieved, "peak": peak,
+                "unit": "GB/s", "frac": achieved / peak, "traffic": traffic, "peak_source": peak_src,
+                "alg_bytes_per_zone": ab["advance"], "kernel_ms": k_ms,
+                "whole_step_frac": ab["step"] * zones / (ms_step * 1e-3) / 1e9 / peak}
+
+    # ---- end to end through the C ABI with HOST buffers (H2D + D2H inside the timed region) --
+    e2e = None
+    need = 2 * ubytes + abytes
+    if not args.no_e2e and host_mem_available() < 1.3 * (need - ubytes) + 8e9:
+        e2e = {"value": None, "unit": UNIT, "skipped": f"host has {host_mem_available() / 1e9:.0f} GB available, "
+               f"needs {need / 1e9:.0f} GB of host buffers"}
+    elif not args.no_e2e:
+        try:
+            A_host = torch.empty(ashape, dtype=torch.float64, pin_memory=pinned)
+            Un_host = torch.empty(ushape, dtype=torch.float64, pin_memory=pinned)
+        except Exception:
+            pinned = False
+            A_host = torch.empty(ashape, dtype=torch.float64)
+            Un_host = torch.empty(ushape, dtype=torch.float64)
+        n_e2e = max(1, min(args.steps, 2))
+        ctx.step_host(U_host, A_host, Un_host, U, U_next, A_new, dt)       # warm-up
+        sync_all()
+        t0 = time.perf_counter()
+        for _ in range(n_e2e):
+            ctx.step_host(U_host, A_host, Un_host, U, U_next, A_new, dt)
+        sync_all()
+        sec = (time.perf_counter() - t0) / n_e2e
+        if world > 1:
+            t = torch.tensor([sec], dtype=torch.float64, device=dev)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            sec = float(t.item())
+        e2e = {"value": zones * world / sec, "unit": UNIT, "h2d_bytes_per_step": ubytes,
+               "d2h_bytes_per_step": abytes + ubytes, "steps": n_e2e, "host_memory": "pinned" if pinned else "pageable",
+               "call": "cst_step_host (H2D U, fill_ghosts, advance_A_update, D2H A and U_next)"}
+        del A_host, Un_host
+
+    cpu_baseline = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        cpu_baseline, _ = time_oracle(cfg, 3, 1)
+
+    if rank == 0:
+        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+                "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
+                "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+                "config": {"workload": f"configs[{cfg['index']}] {cfg['name']}: {cfg['nbx'] * cfg['nby'] * cfg['nbz']} box(es) of "
+                                       f"{cfg['nx']}x{cfg['ny']}x{cfg['nz']}+{cfg['ng']} ghosts, NVAR={N}",
+                           "zones_per_gpu": zones, "step": "fill_ghosts + advance_A_update + cfl_dt_device",
+                           "l2": f"inputs larger than L2 ({(ubytes + 3 * abytes) / 1e9:.1f} GB touched per step)"
+                                 if ubytes > 4e8 else "inputs fit in L2 (debug size)",
+                           "parallelism": f"replicas x{world}" if world > 1 else "single GPU",
+                           "debug_size_override": bool(args.n)},
+                "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline,
+                "cpu_baseline": cpu_baseline}
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

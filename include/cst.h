@@ -1,0 +1,111 @@
+/*
+ * cst.h -- C ABI of the B200-native hot path of Castro's SDC reactive-flow method
+ *          (Zingale et al., arXiv:1910.12578; /root/reference/PAPER.md = "P").
+ *
+ * The library evaluates, on AMReX-style boxes of fp64 conserved state resident in GPU memory,
+ *   S0  ghost-zone fill                        ("grids"/"boxes"; Q16)
+ *   S1-S4  the advective term <A(U)> of Eq. (1) ("the divergence of the hydrodynamic
+ *          fluxes along with hydrodynamic sources"; evaluated at a node time)
+ *   S5  the SDC node update, Eq. (2), R = 0
+ *   S6  the CFL time step                       (BASELINE.json north_star; Q20)
+ * Every step runs in hand-written CUDA kernels for sm_100a; there is no CPU fallback.
+ *
+ * LAYOUT.  All arrays are fp64, C-contiguous, in DEVICE memory:
+ *   U[b][c][k][j][i]  ghosted state, extents nbox x NVAR x (nz+2ng) x (ny+2ng) x (nx+2ng), i fastest
+ *   A[b][c][k][j][i]  interior-only arrays, extents nbox x NVAR x nz x ny x nx
+ *   c = 0 rho, 1 rho*u, 2 rho*v, 3 rho*w, 4 rho*E, 5+s rho*X_s;  NVAR = 5 + nspec
+ *   b = bi + nbx*(bj + nby*bk); box (bi,bj,bk) covers global zones [bi*nx,(bi+1)*nx) x ...
+ *
+ * OWNERSHIP.  The caller owns every state/flux buffer and the stream.  The context owns only a
+ * few KB of device scratch (reduction cells).  No call allocates or frees caller-visible memory.
+ * `stream` is a cudaStream_t passed as void* (NULL = legacy default stream).
+ *
+ * ERRORS.  Every call returns 0 (CST_OK) or a negative code; nothing throws, aborts or prints.
+ * Launches are asynchronous: a device fault surfaces as CST_ECUDA from the next synchronising
+ * call.  NaN / negative-pressure inputs are not detected on the hot path.
+ */
+#ifndef CST_H
+#define CST_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+enum { CST_OK = 0, CST_EINVAL = -1, CST_ECUDA = -2, CST_ENOMEM = -3 };
+enum { CST_BC_PERIODIC = 0, CST_BC_OUTFLOW = 1, CST_BC_REFLECT = 2 };
+#define CST_MAX_QUAD 4      /* at most 4 quadrature nodes in one update (3 used by Simpson)     */
+#define CST_MAX_NSPEC 59    /* NVAR <= 64                                                       */
+
+typedef struct {
+    int    nx, ny, nz;         /* interior zones per box (all boxes equal); each >= ng           */
+    int    ng;                 /* ghost width; must be 4                                         */
+    int    nbx, nby, nbz;      /* box lattice; nbox = nbx*nby*nbz                                */
+    int    nspec;              /* passively advected species; NVAR = 5 + nspec                   */
+    double dx, dy, dz;         /* zone widths (> 0)                                              */
+    double gamma;              /* gamma-law EOS (> 1)                                            */
+    double grav[3];            /* constant acceleration ("hydrodynamic source"); 0 = none */
+    int    bc_lo[3], bc_hi[3]; /* CST_BC_*; periodic must be set on both sides of a direction    */
+    double small_dens, small_pres; /* floors on interface rho, p and zone-centre p (Q11)         */
+} cst_params;
+
+typedef struct cst_ctx cst_ctx;    /* opaque */
+
+/* Validates params (CST_EINVAL: NULL, ng != 4, n_d < ng, nspec out of range, non-positive
+ * widths, gamma <= 1, bad or one-sided-periodic BC) and allocates the context's scratch. */
+int cst_create(const cst_params* params, cst_ctx** out);
+int cst_destroy(cst_ctx* ctx);
+
+/* S0.  Fills the whole 4-deep ghost shell of every box of U in place (faces,
+ * edges, corners) from the interior of the box lattice: neighbour boxes inside the domain,
+ * periodic wrap, outflow = copy of the nearest interior zone, reflecting = mirror image with the
+ * wall-normal momentum negated.  Interior zones are not touched. */
+int cst_fill_ghosts(cst_ctx* ctx, double* U, void* stream);
+
+/* S1-S4.  A <- <A(U)>: conserved->primitive with the gamma-law EOS, PPM
+ * reconstruction (Colella & Woodward 1984 limiter, P:L52 ref [15]) of the primitives in x, y, z,
+ * an HLLC Riemann solve at every face, flux divergence plus the constant-gravity source.
+ * Reads U on the interior and the 3-deep face ghosts (which must be filled); writes all of A. */
+int cst_advance_A(cst_ctx* ctx, const double* U, double* A, void* stream);
+
+/* S5 (Eq. (2) with R = 0).  On interior zones of every box
+ *   U_next = U_m + dt_m*(A_new_m - A_old_m) + sum_{q<nquad} w_quad[q]*A_quad[q]
+ * w_quad (HOST array, weights already multiplied by dt) and A_quad (HOST array of nquad DEVICE
+ * pointers, 0 <= nquad <= CST_MAX_QUAD) are copied by value at the call.  Ghosts of U_next are
+ * left untouched (stale until cst_fill_ghosts).  U_next may alias U_m. */
+int cst_sdc_update(cst_ctx* ctx, double* U_next, const double* U_m, double dt_m,
+                   const double* A_new_m, const double* A_old_m,
+                   int nquad, const double* const* A_quad, const double* w_quad, void* stream);
+
+/* Fused S1-S5: A_new_m <- <A(U_m)> and the node update above with that A_new_m, in one pass over
+ * U_m.  A_old_m or any A_quad[q] may be the A_new_m buffer itself (then they mean the value just
+ * computed, as in the first SDC iteration where every node carries A(U^n)).  U_next must not
+ * alias U_m (CST_EINVAL). */
+int cst_advance_A_update(cst_ctx* ctx, const double* U_m, double* A_new_m, double* U_next,
+                         double dt_m, const double* A_old_m,
+                         int nquad, const double* const* A_quad, const double* w_quad, void* stream);
+
+/* S6 (BASELINE.json north_star; sum form, Q20).
+ *   dt = cfl / max over interior zones of [(|u|+c)/dx + (|v|+c)/dy + (|w|+c)/dz], c = sqrt(gamma p/rho)
+ * cst_cfl_dt_device leaves dt in *dt_out_dev (DEVICE pointer) without synchronising;
+ * cst_cfl_dt writes *dt_out_host (HOST pointer) and synchronises the stream. */
+int cst_cfl_dt_device(cst_ctx* ctx, const double* U, double cfl, double* dt_out_dev, void* stream);
+int cst_cfl_dt(cst_ctx* ctx, const double* U, double cfl, double* dt_out_host, void* stream);
+
+/* Host-buffer convenience used for the end-to-end measurement: copies the interior+ghost array
+ * U_host (HOST, layout of U) to the device buffers owned by the caller (U_dev, U_next_dev,
+ * A_dev), runs fill_ghosts + advance_A_update (forward-Euler node update: A_old = A_quad = A_new)
+ * and copies A and U_next back to A_host / U_next_host.  Synchronises the stream. */
+int cst_step_host(cst_ctx* ctx, const double* U_host, double* A_host, double* U_next_host,
+                  double* U_dev, double* U_next_dev, double* A_dev,
+                  double dt_m, void* stream);
+
+/* Number of kernel launches issued through this context since creation (for bench accounting). */
+long long cst_launch_count(const cst_ctx* ctx);
+
+const char* cst_strerror(int code);   /* static string; for CST_ECUDA the last CUDA error text  */
+const char* cst_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* CST_H */

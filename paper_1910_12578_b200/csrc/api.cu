@@ -1,0 +1,184 @@
+// api.cu -- the C ABI of libcst (include/cst.h): validation, context, argument marshalling.
+// No arithmetic of the method lives here; every step runs in the kernels of this directory.
+#include <new>
+#include <string.h>
+#include "common.cuh"
+
+static thread_local char g_cuda_msg[256] = "no CUDA error recorded";
+
+static int cuda_fail(cudaError_t e)
+{
+    strncpy(g_cuda_msg, cudaGetErrorString(e), sizeof(g_cuda_msg) - 1);
+    g_cuda_msg[sizeof(g_cuda_msg) - 1] = 0;
+    return CST_ECUDA;
+}
+static int check_launch(int rc)
+{
+    if (rc == CST_ECUDA) return cuda_fail(cudaGetLastError());
+    return rc;
+}
+
+static int validate(const cst_params* p)
+{
+    if (!p) return CST_EINVAL;
+    if (p->ng != CST_NG) return CST_EINVAL;
+    if (p->nx < p->ng || p->ny < p->ng || p->nz < p->ng) return CST_EINVAL;
+    if (p->nbx < 1 || p->nby < 1 || p->nbz < 1) return CST_EINVAL;
+    if ((long long)p->nbx * p->nby * p->nbz > 65535) return CST_EINVAL;
+    if (p->nspec < 0 || p->nspec > CST_MAX_NSPEC) return CST_EINVAL;
+    if (!(p->dx > 0) || !(p->dy > 0) || !(p->dz > 0) || !(p->gamma > 1)) return CST_EINVAL;
+    for (int d = 0; d < 3; ++d) {
+        if (p->bc_lo[d] < 0 || p->bc_lo[d] > 2 || p->bc_hi[d] < 0 || p->bc_hi[d] > 2) return CST_EINVAL;
+        if ((p->bc_lo[d] == CST_BC_PERIODIC) != (p->bc_hi[d] == CST_BC_PERIODIC)) return CST_EINVAL;
+    }
+    return CST_OK;
+}
+
+extern "C" int cst_create(const cst_params* p, cst_ctx** out)
+{
+    if (!out) return CST_EINVAL;
+    *out = nullptr;
+    int rc = validate(p);
+    if (rc) return rc;
+    cst_ctx* c = new (std::nothrow) cst_ctx();
+    if (!c) return CST_ENOMEM;
+    c->p = *p;
+    Geom& g = c->g;
+    g.nx = p->nx; g.ny = p->ny; g.nz = p->nz;
+    g.ex = p->nx + 2 * CST_NG; g.ey = p->ny + 2 * CST_NG; g.ez = p->nz + 2 * CST_NG;
+    g.nbx = p->nbx; g.nby = p->nby; g.nbz = p->nbz; g.nbox = p->nbx * p->nby * p->nbz;
+    g.nspec = p->nspec; g.nvar = 5 + p->nspec;
+    for (int d = 0; d < 3; ++d) { g.bc_lo[d] = p->bc_lo[d]; g.bc_hi[d] = p->bc_hi[d]; g.grav[d] = p->grav[d]; }
+    g.dx = p->dx; g.dy = p->dy; g.dz = p->dz;
+    g.rdx = 1.0 / p->dx; g.rdy = 1.0 / p->dy; g.rdz = 1.0 / p->dz;
+    g.gamma = p->gamma; g.gm1 = p->gamma - 1.0; g.rgm1 = 1.0 / (p->gamma - 1.0);
+    g.gfac = (p->gamma + 1.0) / (2.0 * p->gamma);
+    g.small_dens = p->small_dens; g.small_pres = p->small_pres;
+    g.plane_g = (long long)g.ex * g.ey;
+    g.comp_g = g.plane_g * g.ez;
+    g.box_g = g.comp_g * g.nvar;
+    g.comp_a = (long long)g.nx * g.ny * g.nz;
+    g.box_a = g.comp_a * g.nvar;
+    c->launches = 0;
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, dev);
+    if (e == cudaSuccess) e = cudaMalloc(&c->d_scratch, 64 * sizeof(double));
+    if (e != cudaSuccess) { delete c; return cuda_fail(e); }
+    *out = c;
+    return CST_OK;
+}
+
+extern "C" int cst_destroy(cst_ctx* c)
+{
+    if (!c) return CST_EINVAL;
+    cudaFree(c->d_scratch);
+    delete c;
+    return CST_OK;
+}
+
+static int make_quad(int nquad, const double* const* A_quad, const double* w_quad, QuadArgs& q)
+{
+    if (nquad < 0 || nquad > CST_MAX_QUAD) return CST_EINVAL;
+    if (nquad > 0 && (!A_quad || !w_quad)) return CST_EINVAL;
+    q.nquad = nquad;
+    for (int n = 0; n < CST_MAX_QUAD; ++n) { q.A[n] = nullptr; q.w[n] = 0.0; }
+    for (int n = 0; n < nquad; ++n) {
+        if (!A_quad[n]) return CST_EINVAL;
+        q.A[n] = A_quad[n]; q.w[n] = w_quad[n];
+    }
+    return CST_OK;
+}
+
+extern "C" int cst_fill_ghosts(cst_ctx* c, double* U, void* stream)
+{
+    if (!c || !U) return CST_EINVAL;
+    return check_launch(launch_fill_ghosts(c, U, (cudaStream_t)stream));
+}
+
+extern "C" int cst_advance_A(cst_ctx* c, const double* U, double* A, void* stream)
+{
+    if (!c || !U || !A) return CST_EINVAL;
+    QuadArgs q{};
+    return check_launch(launch_advance_A(c, U, A, nullptr, 0.0, nullptr, q, false, (cudaStream_t)stream));
+}
+
+extern "C" int cst_sdc_update(cst_ctx* c, double* U_next, const double* U_m, double dt_m,
+                              const double* A_new_m, const double* A_old_m,
+                              int nquad, const double* const* A_quad, const double* w_quad, void* stream)
+{
+    if (!c || !U_next || !U_m || !A_new_m || !A_old_m) return CST_EINVAL;
+    QuadArgs q;
+    int rc = make_quad(nquad, A_quad, w_quad, q);
+    if (rc) return rc;
+    return check_launch(launch_sdc_update(c, U_next, U_m, dt_m, A_new_m, A_old_m, q, (cudaStream_t)stream));
+}
+
+extern "C" int cst_advance_A_update(cst_ctx* c, const double* U_m, double* A_new_m, double* U_next,
+                                    double dt_m, const double* A_old_m,
+                                    int nquad, const double* const* A_quad, const double* w_quad, void* stream)
+{
+    if (!c || !U_m || !A_new_m || !U_next || !A_old_m) return CST_EINVAL;
+    if (U_next == U_m) return CST_EINVAL;
+    QuadArgs q;
+    int rc = make_quad(nquad, A_quad, w_quad, q);
+    if (rc) return rc;
+    return check_launch(launch_advance_A(c, U_m, A_new_m, U_next, dt_m, A_old_m, q, true, (cudaStream_t)stream));
+}
+
+extern "C" int cst_cfl_dt_device(cst_ctx* c, const double* U, double cfl, double* dt_out_dev, void* stream)
+{
+    if (!c || !U || !dt_out_dev || !(cfl > 0)) return CST_EINVAL;
+    return check_launch(launch_cfl(c, U, cfl, dt_out_dev, (cudaStream_t)stream));
+}
+
+extern "C" int cst_cfl_dt(cst_ctx* c, const double* U, double cfl, double* dt_out_host, void* stream)
+{
+    if (!c || !U || !dt_out_host || !(cfl > 0)) return CST_EINVAL;
+    cudaStream_t st = (cudaStream_t)stream;
+    int rc = check_launch(launch_cfl(c, U, cfl, c->d_scratch + 1, st));
+    if (rc) return rc;
+    cudaError_t e = cudaMemcpyAsync(dt_out_host, c->d_scratch + 1, sizeof(double), cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    return e == cudaSuccess ? CST_OK : cuda_fail(e);
+}
+
+extern "C" int cst_step_host(cst_ctx* c, const double* U_host, double* A_host, double* U_next_host,
+                             double* U_dev, double* U_next_dev, double* A_dev, double dt_m, void* stream)
+{
+    if (!c || !U_host || !A_host || !U_next_host || !U_dev || !U_next_dev || !A_dev) return CST_EINVAL;
+    if (U_dev == U_next_dev) return CST_EINVAL;
+    cudaStream_t st = (cudaStream_t)stream;
+    const Geom& g = c->g;
+    const size_t ub = (size_t)g.box_g * g.nbox * sizeof(double), ab = (size_t)g.box_a * g.nbox * sizeof(double);
+    cudaError_t e = cudaMemcpyAsync(U_dev, U_host, ub, cudaMemcpyHostToDevice, st);
+    if (e != cudaSuccess) return cuda_fail(e);
+    // U_next starts as a copy of U_m so that its ghost shell is defined (stale, as documented)
+    e = cudaMemcpyAsync(U_next_dev, U_dev, ub, cudaMemcpyDeviceToDevice, st);
+    if (e != cudaSuccess) return cuda_fail(e);
+    int rc = check_launch(launch_fill_ghosts(c, U_dev, st));
+    if (rc) return rc;
+    QuadArgs q{};
+    q.nquad = 2; q.A[0] = A_dev; q.A[1] = A_dev; q.w[0] = 0.5 * dt_m; q.w[1] = 0.5 * dt_m;
+    rc = check_launch(launch_advance_A(c, U_dev, A_dev, U_next_dev, dt_m, A_dev, q, true, st));
+    if (rc) return rc;
+    e = cudaMemcpyAsync(A_host, A_dev, ab, cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(U_next_host, U_next_dev, ub, cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    return e == cudaSuccess ? CST_OK : cuda_fail(e);
+}
+
+extern "C" long long cst_launch_count(const cst_ctx* c) { return c ? c->launches : -1; }
+
+extern "C" const char* cst_strerror(int code)
+{
+    switch (code) {
+    case CST_OK: return "ok";
+    case CST_EINVAL: return "invalid argument";
+    case CST_ECUDA: return g_cuda_msg;
+    case CST_ENOMEM: return "out of host memory";
+    default: return "unknown error code";
+    }
+}
+
+extern "C" const char* cst_version(void) { return "libcst 0.1 (sm_100a)"; }

@@ -1,0 +1,57 @@
+// common.cuh -- geometry shared by the CUDA kernels of libcst (product code; shares nothing
+// with oracle/).  Layout and index conventions: include/cst.h, DESIGN.md section 4.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include "../../include/cst.h"
+
+#define CST_NG 4
+
+struct Geom {
+    int nx, ny, nz;          // interior zones per box
+    int ex, ey, ez;          // ghosted extents
+    int nbx, nby, nbz, nbox;
+    int nspec, nvar;
+    int bc_lo[3], bc_hi[3];
+    double dx, dy, dz;
+    double rdx, rdy, rdz;    // reciprocals
+    double gamma, gm1, rgm1, gfac;   // gamma, gamma-1, 1/(gamma-1), (gamma+1)/(2 gamma)
+    double grav[3];
+    double small_dens, small_pres;
+    long long plane_g;       // ex*ey
+    long long comp_g;        // ex*ey*ez   (stride between components of U)
+    long long box_g;         // nvar*comp_g
+    long long comp_a;        // nx*ny*nz   (stride between components of A)
+    long long box_a;         // nvar*comp_a
+};
+
+struct cst_ctx {
+    cst_params p;
+    Geom g;
+    double* d_scratch;       // [0] = max signal rate bits, [1] = dt
+    long long launches;
+    int sm_count;
+};
+
+struct QuadArgs {            // passed by value to the update kernels
+    int nquad;
+    const double* A[CST_MAX_QUAD];
+    double w[CST_MAX_QUAD];
+};
+
+__host__ __device__ inline long long uidx(const Geom& g, int b, int c, int k, int j, int i)
+{   // ghosted index; k, j, i in [0, e*)
+    return (long long)b * g.box_g + (long long)c * g.comp_g + ((long long)k * g.ey + j) * g.ex + i;
+}
+__host__ __device__ inline long long aidx(const Geom& g, int b, int c, int k, int j, int i)
+{   // interior index; k, j, i in [0, n*)
+    return (long long)b * g.box_a + (long long)c * g.comp_a + ((long long)k * g.ny + j) * g.nx + i;
+}
+
+// launchers (one per source file)
+int launch_fill_ghosts(cst_ctx*, double* U, cudaStream_t);
+int launch_advance_A(cst_ctx*, const double* U, double* A, double* U_next, double dt_m,
+                     const double* A_old_m, const QuadArgs& q, bool fused, cudaStream_t);
+int launch_sdc_update(cst_ctx*, double* U_next, const double* U_m, double dt_m,
+                      const double* A_new_m, const double* A_old_m, const QuadArgs& q, cudaStream_t);
+int launch_cfl(cst_ctx*, const double* U, double cfl, double* dt_out_dev, cudaStream_t);
