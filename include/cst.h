@@ -16,8 +16,9 @@
  *   c = 0 rho, 1 rho*u, 2 rho*v, 3 rho*w, 4 rho*E, 5+s rho*X_s;  NVAR = 5 + nspec
  *   b = bi + nbx*(bj + nby*bk); box (bi,bj,bk) covers global zones [bi*nx,(bi+1)*nx) x ...
  *
- * OWNERSHIP.  The caller owns every state/flux buffer and the stream.  The context owns only a
- * few KB of device scratch (reduction cells).  No call allocates or frees caller-visible memory.
+ * OWNERSHIP.  The caller owns every state/flux buffer, the workspace and the stream.  The context
+ * owns only a few KB of device scratch (reduction cells).  No call allocates or frees device memory
+ * after cst_create.
  * `stream` is a cudaStream_t passed as void* (NULL = legacy default stream).
  *
  * ERRORS.  Every call returns 0 (CST_OK) or a negative code; nothing throws, aborts or prints.
@@ -31,7 +32,7 @@
 extern "C" {
 #endif
 
-enum { CST_OK = 0, CST_EINVAL = -1, CST_ECUDA = -2, CST_ENOMEM = -3 };
+enum { CST_OK = 0, CST_EINVAL = -1, CST_ECUDA = -2, CST_ENOMEM = -3, CST_ENOWORKSPACE = -4 };
 enum { CST_BC_PERIODIC = 0, CST_BC_OUTFLOW = 1, CST_BC_REFLECT = 2 };
 #define CST_MAX_QUAD 4      /* at most 4 quadrature nodes in one update (3 used by Simpson)     */
 #define CST_MAX_NSPEC 59    /* NVAR <= 64                                                       */
@@ -54,6 +55,15 @@ typedef struct cst_ctx cst_ctx;    /* opaque */
  * widths, gamma <= 1, bad or one-sided-periodic BC) and allocates the context's scratch. */
 int cst_create(const cst_params* params, cst_ctx** out);
 int cst_destroy(cst_ctx* ctx);
+
+/* Workspace of cst_advance_A / cst_advance_A_update / cst_step_host.  <A(U)> is evaluated by a hydro
+ * kernel and a species kernel (F(rho X_s) = F(rho) * upwind X_s); the face mass fluxes F(rho) and
+ * 1/rho travel between them through a caller-owned DEVICE buffer of cst_workspace_bytes() bytes
+ * (about 34 bytes per ghosted zone; 16-byte aligned; contents are scratch, valid only within one
+ * call).  cst_set_workspace stores the pointer (CST_EINVAL if NULL or too small); the advance calls
+ * return CST_ENOWORKSPACE until it has been set.  One workspace serves one stream at a time. */
+long long cst_workspace_bytes(const cst_ctx* ctx);
+int cst_set_workspace(cst_ctx* ctx, void* workspace_dev, long long bytes);
 
 /* S0.  Fills the whole 4-deep ghost shell of every box of U in place (faces,
  * edges, corners) from the interior of the box lattice: neighbour boxes inside the domain,
@@ -97,7 +107,7 @@ int cst_cfl_dt(cst_ctx* ctx, const double* U, double cfl, double* dt_out_host, v
  * and copies A and U_next back to A_host / U_next_host.  Synchronises the stream. */
 int cst_step_host(cst_ctx* ctx, const double* U_host, double* A_host, double* U_next_host,
                   double* U_dev, double* U_next_dev, double* A_dev,
-                  double dt_m, void* stream);
+                  double dt_m, void* stream);   /* needs the workspace, see cst_set_workspace */
 
 /* Number of kernel launches issued through this context since creation (for bench accounting). */
 long long cst_launch_count(const cst_ctx* ctx);

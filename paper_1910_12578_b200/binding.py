@@ -11,7 +11,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libcst.so")
 MAX_QUAD = 4
 
-EXPORTS = ["cst_create", "cst_destroy", "cst_fill_ghosts", "cst_advance_A", "cst_sdc_update",
+EXPORTS = ["cst_create", "cst_destroy", "cst_workspace_bytes", "cst_set_workspace", "cst_fill_ghosts", "cst_advance_A", "cst_sdc_update",
            "cst_advance_A_update", "cst_cfl_dt_device", "cst_cfl_dt", "cst_step_host",
            "cst_launch_count", "cst_strerror", "cst_version"]
 
@@ -47,6 +47,9 @@ def load():
     P = C.POINTER(CstParams)
     lib.cst_create.argtypes = [P, C.POINTER(_vp)]
     lib.cst_destroy.argtypes = [_vp]
+    lib.cst_workspace_bytes.argtypes = [_vp]
+    lib.cst_workspace_bytes.restype = C.c_longlong
+    lib.cst_set_workspace.argtypes = [_vp, _vp, C.c_longlong]
     lib.cst_fill_ghosts.argtypes = [_vp, _vp, _vp]
     lib.cst_advance_A.argtypes = [_vp, _vp, _vp, _vp]
     lib.cst_sdc_update.argtypes = [_vp, _vp, _vp, C.c_double, _vp, _vp, C.c_int, C.POINTER(_vp), _dp, _vp]
@@ -97,11 +100,29 @@ def _stream(stream):
 class Context:
     """Owns one cst_ctx.  Methods mirror the C entry points (same names, same argument order)."""
 
-    def __init__(self, cfg):
+    def __init__(self, cfg, workspace="auto"):
+        """workspace="auto": a torch uint8 tensor of workspace_bytes() is allocated on the current CUDA
+        device and handed to cst_set_workspace (the library itself never allocates it);
+        workspace=None: the caller calls set_workspace() later."""
         self.lib = load()
         self.cfg = dict(cfg)
         self._h = _vp()
+        self._ws = None
         self._check(self.lib.cst_create(C.byref(make_params(cfg)), C.byref(self._h)), "cst_create")
+        if workspace == "auto":
+            import torch
+            self.set_workspace(torch.empty(self.workspace_bytes(), dtype=torch.uint8, device="cuda"))
+        elif workspace is not None:
+            self.set_workspace(workspace)
+
+    def workspace_bytes(self):
+        return int(self.lib.cst_workspace_bytes(self._h))
+
+    def set_workspace(self, buf):
+        """buf: contiguous torch CUDA tensor (any dtype) of at least workspace_bytes() bytes; kept alive here."""
+        nbytes = buf.numel() * buf.element_size()
+        self._check(self.lib.cst_set_workspace(self._h, buf.data_ptr(), nbytes), "cst_set_workspace")
+        self._ws = buf
 
     def _check(self, rc, what):
         if rc != 0:

@@ -1,0 +1,175 @@
+// advect_hydro.cu -- S1-S4 (+ fused S5) for the five hydrodynamic components (rho, rho u, rho v,
+// rho w, rho E) of <A(U)> (include/cst.h cst_advance_A).
+//
+// One CTA = one 16^3 tile (tile.cuh).  Three sweeps, x then y then z.  In each sweep a thread marches
+// along its pencil: it loads the conserved state of the next zone, converts it to primitives
+// (S1), slides five PPM windows (S2, sweep.cuh), solves the HLLC problem at the face that has
+// just become complete (S3) and differences consecutive face fluxes (S4).  Every face flux and
+// every parabola of the tile is therefore computed once.  The x and y contributions to A are
+// accumulated in shared memory (5 x 16^3 doubles); the z sweep adds its own, the gravity source and
+// writes A (and, fused, the SDC node update S5).
+// Side products for the species kernel: 1/rho of every zone the species stencil touches (workspace
+// rinv) and the mass flux F(rho) of every face (workspace Fm, thread-private slots, tile.cuh).
+#include "sweep.cuh"
+#include "tile.cuh"
+
+#define PART_PITCH 17                                  // odd pitch: conflict-free for every sweep
+#define PART_COMP (TILE * TILE * PART_PITCH)           // doubles per component
+
+template <int D>
+__device__ __forceinline__ void hydro_sweep(const Geom& g, const TileCoord& tc, const double* __restrict__ Ub,
+                                            double* __restrict__ part, double* __restrict__ fm_tile,
+                                            double* __restrict__ rinv_b, double* __restrict__ A,
+                                            const UpdArgs& up)
+{
+    const int ng = CST_NG;
+    const int tid = threadIdx.x, a = tid & (TILE - 1), b = tid >> 4;
+    int L, ea, eb;
+    if (D == 0) { L = tc.tx; ea = tc.ty; eb = tc.tz; }
+    else if (D == 1) { L = tc.ty; ea = tc.tx; eb = tc.tz; }
+    else { L = tc.tz; ea = tc.tx; eb = tc.ty; }
+    if (a >= ea || b >= eb) return;
+
+    // ghosted linear index of pencil position p = 0 and the stride along the pencil
+    long long z0, stride;
+    int n_d, o_d;
+    if (D == 0) {
+        z0 = ((long long)(tc.k0 + b + ng) * g.ey + (tc.j0 + a + ng)) * g.ex + (tc.i0 + ng);
+        stride = 1; n_d = g.nx; o_d = tc.i0;
+    } else if (D == 1) {
+        z0 = ((long long)(tc.k0 + b + ng) * g.ey + (tc.j0 + ng)) * g.ex + (tc.i0 + a + ng);
+        stride = g.ex; n_d = g.ny; o_d = tc.j0;
+    } else {
+        z0 = ((long long)(tc.k0 + ng) * g.ey + (tc.j0 + b + ng)) * g.ex + (tc.i0 + a + ng);
+        stride = g.plane_g; n_d = g.nz; o_d = tc.k0;
+    }
+    const bool ghost_lo = (o_d == 0), ghost_hi = (o_d + L == n_d);
+    const double rd = (D == 0) ? g.rdx : (D == 1) ? g.rdy : g.rdz;
+
+    PpmWindow w[5];
+    double Uc[5], Fprev[5];
+#pragma unroll
+    for (int c = 0; c < 5; ++c) Uc[c] = Ub[c * g.comp_g + z0 - 3 * stride];
+
+    for (int p = -3; p <= L + 2; ++p) {
+        // prefetch the next zone of the pencil while this one is processed
+        double Un[5];
+        if (p < L + 2) {
+            const long long zn = z0 + (long long)(p + 1) * stride;
+#pragma unroll
+            for (int c = 0; c < 5; ++c) Un[c] = Ub[c * g.comp_g + zn];
+        }
+        double W[5];
+        const double r = cons_to_prim(g, Uc[0], Uc[1], Uc[2], Uc[3], Uc[4], W);
+        if ((D == 2 && p >= 0 && p < L) || (p < 0 && ghost_lo) || (p >= L && ghost_hi))
+            rinv_b[z0 + (long long)p * stride] = r;
+
+        if (p == -3) {
+#pragma unroll
+            for (int c = 0; c < 5; ++c) w[c].start(W[c]);
+        } else if (p == -2) {
+#pragma unroll
+            for (int c = 0; c < 5; ++c) w[c].warm1(W[c]);
+        } else if (p == -1) {
+#pragma unroll
+            for (int c = 0; c < 5; ++c) w[c].warm2(W[c]);
+        } else if (p == 0) {
+#pragma unroll
+            for (int c = 0; c < 5; ++c) w[c].warm3(W[c]);
+        } else {
+#pragma unroll
+            for (int c = 0; c < 5; ++c) w[c].push(W[c]);
+            if (p >= 2) {
+                // face f = p-2 between zones p-3 and p-2
+                double WL[5], WR[5], F[5];
+#pragma unroll
+                for (int c = 0; c < 5; ++c) { WL[c] = w[c].qpL; WR[c] = w[c].qm; }
+                WL[0] = fmax(WL[0], g.small_dens); WR[0] = fmax(WR[0], g.small_dens);
+                WL[4] = fmax(WL[4], g.small_pres); WR[4] = fmax(WR[4], g.small_pres);
+                hllc<D>(g, WL, WR, F);
+                fm_tile[((D * (TILE + 1)) + (p - 2)) * NTHR + tid] = F[0];
+                if (p >= 3) {
+                    const int q = p - 3;                     // zone of the pencil that is now complete
+                    int li, lj, lk;
+                    if (D == 0) { li = q; lj = a; lk = b; }
+                    else if (D == 1) { li = a; lj = q; lk = b; }
+                    else { li = a; lj = b; lk = q; }
+                    const int sp = (lk * TILE + lj) * PART_PITCH + li;
+                    if (D == 0) {
+#pragma unroll
+                        for (int c = 0; c < 5; ++c) part[c * PART_COMP + sp] = -(F[c] - Fprev[c]) * rd;
+                    } else if (D == 1) {
+#pragma unroll
+                        for (int c = 0; c < 5; ++c)
+                            part[c * PART_COMP + sp] = fma(-(F[c] - Fprev[c]), rd, part[c * PART_COMP + sp]);
+                    } else {
+                        double A5[5];
+#pragma unroll
+                        for (int c = 0; c < 5; ++c) A5[c] = fma(-(F[c] - Fprev[c]), rd, part[c * PART_COMP + sp]);
+                        const long long zc = z0 + (long long)q * stride;
+                        const bool grav = (g.grav[0] != 0.0) || (g.grav[1] != 0.0) || (g.grav[2] != 0.0);
+                        double Um[5];
+                        if (grav || up.fused) {
+#pragma unroll
+                            for (int c = 0; c < 5; ++c) Um[c] = Ub[c * g.comp_g + zc];
+                        }
+                        if (grav) {     // S4 source: constant gravity from the zone-centre state
+                            A5[1] = fma(Um[0], g.grav[0], A5[1]);
+                            A5[2] = fma(Um[0], g.grav[1], A5[2]);
+                            A5[3] = fma(Um[0], g.grav[2], A5[3]);
+                            A5[4] += fma(Um[3], g.grav[2], fma(Um[2], g.grav[1], Um[1] * g.grav[0]));
+                        }
+                        const long long ia0 = (long long)tc.b * g.box_a +
+                            ((long long)(tc.k0 + lk) * g.ny + (tc.j0 + lj)) * g.nx + (tc.i0 + li);
+#pragma unroll
+                        for (int c = 0; c < 5; ++c) {
+                            const long long ia = ia0 + c * g.comp_a;
+                            if (up.fused)
+                                up.U_next[(long long)tc.b * g.box_g + c * g.comp_g + zc] =
+                                    node_update(up, Um[c], A5[c], ia);
+                            A[ia] = A5[c];
+                        }
+                    }
+                }
+#pragma unroll
+                for (int c = 0; c < 5; ++c) Fprev[c] = F[c];
+            }
+        }
+#pragma unroll
+        for (int c = 0; c < 5; ++c) Uc[c] = Un[c];
+    }
+}
+
+__global__ void __launch_bounds__(NTHR, 1)
+k_advect_hydro(Geom g, TileGeom tg, const double* __restrict__ U, double* __restrict__ A,
+               double* __restrict__ rinv, double* __restrict__ Fm, UpdArgs up)
+{
+    extern __shared__ double part[];                   // [5][TILE][TILE][PART_PITCH]
+    const TileCoord tc = tile_coord(g, tg, blockIdx.x);
+    const double* Ub = U + (long long)tc.b * g.box_g;
+    double* rinv_b = rinv + (long long)tc.b * g.comp_g;
+    double* fm_tile = Fm + tc.tile * 3LL * (TILE + 1) * NTHR;
+    hydro_sweep<0>(g, tc, Ub, part, fm_tile, rinv_b, A, up);
+    __syncthreads();
+    hydro_sweep<1>(g, tc, Ub, part, fm_tile, rinv_b, A, up);
+    __syncthreads();
+    hydro_sweep<2>(g, tc, Ub, part, fm_tile, rinv_b, A, up);
+}
+
+int launch_advect_hydro(cst_ctx* ctx, const double* U, double* A, const UpdArgs& up, cudaStream_t st)
+{
+    const Geom& g = ctx->g;
+    const TileGeom tg = make_tile_geom(g);
+    const size_t smem = 5ull * PART_COMP * sizeof(double);
+    static bool attr_set = false;
+    if (!attr_set) {
+        if (cudaFuncSetAttribute(k_advect_hydro, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
+            return CST_ECUDA;
+        attr_set = true;
+    }
+    double* rinv = ctx->ws;
+    double* Fm = ctx->ws + ws_rinv_doubles(g);
+    k_advect_hydro<<<(unsigned)tg.ntiles, NTHR, smem, st>>>(g, tg, U, A, rinv, Fm, up);
+    ctx->launches++;
+    return cudaGetLastError() == cudaSuccess ? CST_OK : CST_ECUDA;
+}

@@ -60,6 +60,7 @@ extern "C" int cst_create(const cst_params* p, cst_ctx** out)
     g.comp_a = (long long)g.nx * g.ny * g.nz;
     g.box_a = g.comp_a * g.nvar;
     c->launches = 0;
+    c->ws = nullptr; c->ws_bytes = 0;
     int dev = 0;
     cudaError_t e = cudaGetDevice(&dev);
     if (e == cudaSuccess) e = cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, dev);
@@ -74,6 +75,18 @@ extern "C" int cst_destroy(cst_ctx* c)
     if (!c) return CST_EINVAL;
     cudaFree(c->d_scratch);
     delete c;
+    return CST_OK;
+}
+
+extern "C" long long cst_workspace_bytes(const cst_ctx* c)
+{
+    return c ? workspace_bytes(c->g) : -1;
+}
+
+extern "C" int cst_set_workspace(cst_ctx* c, void* ws, long long bytes)
+{
+    if (!c || !ws || bytes < workspace_bytes(c->g) || ((uintptr_t)ws & 15)) return CST_EINVAL;
+    c->ws = (double*)ws; c->ws_bytes = bytes;
     return CST_OK;
 }
 
@@ -177,8 +190,9 @@ extern "C" const char* cst_strerror(int code)
     case CST_EINVAL: return "invalid argument";
     case CST_ECUDA: return g_cuda_msg;
     case CST_ENOMEM: return "out of host memory";
+    case CST_ENOWORKSPACE: return "workspace not set (cst_set_workspace)";
     default: return "unknown error code";
     }
 }
 
-extern "C" const char* cst_version(void) { return "libcst 0.1 (sm_100a)"; }
+extern "C" const char* cst_version(void) { return "libcst 0.2 (sm_100a)"; }

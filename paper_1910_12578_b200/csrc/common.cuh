@@ -29,10 +29,13 @@ struct cst_ctx {
     cst_params p;
     Geom g;
     double* d_scratch;       // [0] = max signal rate bits, [1] = dt
+    double* ws;              // caller-owned workspace (cst_set_workspace): [rinv][Fm], tile.cuh
+    long long ws_bytes;
     long long launches;
     int sm_count;
 };
 
+struct UpdArgs;
 struct QuadArgs {            // passed by value to the update kernels
     int nquad;
     const double* A[CST_MAX_QUAD];
@@ -52,6 +55,9 @@ __host__ __device__ inline long long aidx(const Geom& g, int b, int c, int k, in
 int launch_fill_ghosts(cst_ctx*, double* U, cudaStream_t);
 int launch_advance_A(cst_ctx*, const double* U, double* A, double* U_next, double dt_m,
                      const double* A_old_m, const QuadArgs& q, bool fused, cudaStream_t);
+int launch_advect_hydro(cst_ctx*, const double* U, double* A, const UpdArgs& up, cudaStream_t);
+int launch_advect_species(cst_ctx*, const double* U, double* A, const UpdArgs& up, cudaStream_t);
+long long workspace_bytes(const Geom& g);
 int launch_sdc_update(cst_ctx*, double* U_next, const double* U_m, double dt_m,
                       const double* A_new_m, const double* A_old_m, const QuadArgs& q, cudaStream_t);
 int launch_cfl(cst_ctx*, const double* U, double cfl, double* dt_out_dev, cudaStream_t);

@@ -1,0 +1,82 @@
+// tile.cuh -- tiling of a box into 16^3-zone tiles and the pencil <-> thread map shared by the
+// hydro and species kernels of <A(U)>.
+//
+// One CTA of 256 threads owns one tile of up to 16 x 16 x 16 interior zones of one box.  In the
+// sweep along direction d every thread owns one PENCIL of the tile (a line of zones along d) and
+// marches along it with the PPM stencil in a register window:
+//     x sweep: thread (a, b) = (j, k)      y sweep: (a, b) = (i, k)      z sweep: (a, b) = (i, j)
+// with a = tid % 16, b = tid / 16.  The face mass fluxes F(rho) that couple the species to the
+// hydro are exchanged through a THREAD-PRIVATE slot array in the workspace:
+//     Fm[((tile * 3 + d) * (TILE + 1) + f) * NTHR + tid],   f = 0 .. L  (face f lies between zones f-1, f)
+// which is written and read with the same thread map, so every access is fully coalesced.
+#pragma once
+#include "common.cuh"
+
+#define TILE 16
+#define NTHR 256
+
+struct TileGeom {
+    int ntx, nty, ntz;        // tiles per box in each direction
+    int tiles_per_box;
+    long long ntiles;         // nbox * tiles_per_box
+};
+
+__host__ __device__ inline TileGeom make_tile_geom(const Geom& g)
+{
+    TileGeom t;
+    t.ntx = (g.nx + TILE - 1) / TILE;
+    t.nty = (g.ny + TILE - 1) / TILE;
+    t.ntz = (g.nz + TILE - 1) / TILE;
+    t.tiles_per_box = t.ntx * t.nty * t.ntz;
+    t.ntiles = (long long)g.nbox * t.tiles_per_box;
+    return t;
+}
+
+// workspace layout (doubles): [ rinv : nbox * comp_g ][ Fm : ntiles * 3 * (TILE+1) * NTHR ]
+__host__ __device__ inline long long ws_rinv_doubles(const Geom& g) { return (long long)g.nbox * g.comp_g; }
+__host__ __device__ inline long long ws_fm_doubles(const Geom& g)
+{
+    return make_tile_geom(g).ntiles * 3LL * (TILE + 1) * NTHR;
+}
+
+struct TileCoord {
+    int b;                    // box
+    int i0, j0, k0;           // interior origin of the tile inside the box
+    int tx, ty, tz;           // extents (<= TILE)
+    long long tile;           // global tile index
+};
+
+__device__ __forceinline__ TileCoord tile_coord(const Geom& g, const TileGeom& tg, long long tile)
+{
+    TileCoord t;
+    t.tile = tile;
+    t.b = (int)(tile / tg.tiles_per_box);
+    int r = (int)(tile - (long long)t.b * tg.tiles_per_box);
+    const int tk = r / (tg.ntx * tg.nty);
+    r -= tk * tg.ntx * tg.nty;
+    const int tj = r / tg.ntx, ti = r - tj * tg.ntx;
+    t.i0 = ti * TILE; t.j0 = tj * TILE; t.k0 = tk * TILE;
+    t.tx = min(TILE, g.nx - t.i0); t.ty = min(TILE, g.ny - t.j0); t.tz = min(TILE, g.nz - t.k0);
+    return t;
+}
+
+struct UpdArgs {              // the SDC node update fused behind A (S5); see include/cst.h
+    bool fused;
+    double* U_next;
+    double dt_m;
+    const double* A_old;      // nullptr = "the value just computed"
+    int nquad;
+    const double* Aq[CST_MAX_QUAD];   // nullptr = "the value just computed"
+    double w[CST_MAX_QUAD];
+};
+
+// U_next = U_m + dt_m (A_new - A_old) + sum_q w_q A_q   (Eq. (2) of the paper, R = 0)
+__device__ __forceinline__ double node_update(const UpdArgs& up, double um, double a, long long ia)
+{
+    const double aold = up.A_old ? up.A_old[ia] : a;
+    double acc = 0.0;
+#pragma unroll
+    for (int q = 0; q < CST_MAX_QUAD; ++q)
+        if (q < up.nquad) acc = fma(up.w[q], up.Aq[q] ? up.Aq[q][ia] : a, acc);
+    return fma(up.dt_m, a - aold, um) + acc;
+}
