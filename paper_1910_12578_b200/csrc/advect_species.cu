@@ -36,7 +36,7 @@ __device__ __forceinline__ void species_sweep(const Geom& g, const TileCoord& tc
         stride = 1; s0 = (b * TILE + a) * SP_PITCH; sstride = 1;
     } else if (D == 1) {
         z0 = ((long long)(tc.k0 + b + ng) * g.ey + (tc.j0 + ng)) * g.ex + (tc.i0 + a + ng);
-        stride = g.ex; s0 = (b * TILE * TILE) * SP_PITCH + a; sstride = SP_PITCH;
+        stride = g.ex; s0 = (b * TILE) * SP_PITCH + a; sstride = SP_PITCH;
     } else {
         z0 = ((long long)(tc.k0 + ng) * g.ey + (tc.j0 + b + ng)) * g.ex + (tc.i0 + a + ng);
         stride = g.plane_g; s0 = b * SP_PITCH + a; sstride = TILE * SP_PITCH;
