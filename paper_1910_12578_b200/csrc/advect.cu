@@ -11,18 +11,37 @@ long long workspace_bytes(const Geom& g)
     return (ws_rinv_doubles(g) + ws_fm_doubles(g)) * (long long)sizeof(double);
 }
 
+// Eq. (2) with R = 0 -> coefficient list (tile.cuh UpdArgs).  Returns false when more than
+// UPD_MAX_EXT distinct external arrays are involved.
+static bool make_upd(UpdArgs& up, const double* U, double* A, double* U_next, double dt_m,
+                     const double* A_old_m, const QuadArgs& q)
+{
+    up.nr = 0; up.U_m = U; up.U_next = U_next; up.ca = 0.0;
+    for (int r = 0; r < UPD_MAX_EXT; ++r) { up.P[r] = nullptr; up.c[r] = 0.0; }
+    auto add = [&](const double* ptr, double coef) -> bool {
+        if (ptr == A) { up.ca += coef; return true; }
+        for (int r = 0; r < up.nr; ++r) if (up.P[r] == ptr) { up.c[r] += coef; return true; }
+        if (up.nr == UPD_MAX_EXT) return false;
+        up.P[up.nr] = ptr; up.c[up.nr] = coef; up.nr++;
+        return true;
+    };
+    bool ok = add(A, dt_m) && add(A_old_m, -dt_m);
+    for (int n = 0; ok && n < q.nquad; ++n) ok = add(q.A[n], q.w[n]);
+    return ok;
+}
+
 int launch_advance_A(cst_ctx* ctx, const double* U, double* A, double* U_next, double dt_m,
                      const double* A_old_m, const QuadArgs& q, bool fused, cudaStream_t st)
 {
     if (!ctx->ws || ctx->ws_bytes < workspace_bytes(ctx->g)) return CST_ENOWORKSPACE;
     UpdArgs up{};
-    up.fused = fused;
-    up.U_next = U_next;
-    up.dt_m = dt_m;
-    up.A_old = (A_old_m == A) ? nullptr : A_old_m;
-    up.nquad = fused ? q.nquad : 0;
-    for (int n = 0; n < up.nquad; ++n) { up.Aq[n] = (q.A[n] == A) ? nullptr : q.A[n]; up.w[n] = q.w[n]; }
+    up.nr = -1; up.U_m = U;
+    bool split = false;
+    if (fused && !make_upd(up, U, A, U_next, dt_m, A_old_m, q)) { up.nr = -1; split = true; }
     int rc = launch_advect_hydro(ctx, U, A, up, st);
     if (rc) return rc;
-    return launch_advect_species(ctx, U, A, up, st);
+    rc = launch_advect_species(ctx, U, A, up, st);
+    if (rc || !split) return rc;
+    // too many distinct arrays for the fused epilogue: A first, then the plain update kernel
+    return launch_sdc_update(ctx, U_next, U, dt_m, A, A_old_m, q, st);
 }

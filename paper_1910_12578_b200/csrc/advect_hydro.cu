@@ -10,13 +10,183 @@
 // writes A (and, fused, the SDC node update S5).
 // Side products for the species kernel: 1/rho of every zone the species stencil touches (workspace
 // rinv) and the mass flux F(rho) of every face (workspace Fm, thread-private slots, tile.cuh).
+//
+// Two bodies of the same arithmetic: hydro_sweep_full (full 16^3 tile: march unrolled at compile
+// time, the x sweep reads 32-byte groups of four zones so that every fetched sector is used) and
+// hydro_sweep (any tile extent).
 #include "sweep.cuh"
 #include "tile.cuh"
 
 #define PART_PITCH 17                                  // odd pitch: conflict-free for every sweep
 #define PART_COMP (TILE * TILE * PART_PITCH)           // doubles per component
 
-template <int D>
+// ------------------------------------------------------------------------ full 16^3 tiles ----
+__device__ __forceinline__ void ldg256(const double* p, double v[4])
+{   // one 32-byte sector per thread (p is 32-byte aligned)
+    asm volatile("ld.global.nc.v4.f64 {%0,%1,%2,%3}, [%4];"
+                 : "=d"(v[0]), "=d"(v[1]), "=d"(v[2]), "=d"(v[3]) : "l"(p));
+}
+
+struct HydroMarch {           // per-thread state of one pencil march
+    PpmWindow w[5];
+    double Fprev[5];
+};
+
+// one zone of the march: pencil position P (compile-time after unrolling), conserved state Uc
+template <int D, int NR>
+__device__ __forceinline__ void hydro_zone(const Geom& g, const TileCoord& tc, HydroMarch& m, const int p,
+                                           const double Uc[5], const double* __restrict__ Ub,
+                                           double* __restrict__ part, double* __restrict__ fm_slot,
+                                           double* __restrict__ rinv_b, double* __restrict__ A, const UpdArgs& up,
+                                           const long long z0, const long long stride, const bool ghost_lo,
+                                           const bool ghost_hi, const int a, const int b)
+{
+    constexpr int L = TILE;
+    const double nrd = -((D == 0) ? g.rdx : (D == 1) ? g.rdy : g.rdz);
+    double W[5];
+    const double r = cons_to_prim(g, Uc[0], Uc[1], Uc[2], Uc[3], Uc[4], W);
+    if ((D == 2 && p >= 0 && p < L) || (p < 0 && ghost_lo) || (p >= L && ghost_hi))
+        rinv_b[z0 + (long long)p * stride] = r;
+    if (p == -3) {
+#pragma unroll
+        for (int c = 0; c < 5; ++c) m.w[c].start(W[c]);
+    } else if (p == -2) {
+#pragma unroll
+        for (int c = 0; c < 5; ++c) m.w[c].warm1(W[c]);
+    } else if (p == -1) {
+#pragma unroll
+        for (int c = 0; c < 5; ++c) m.w[c].warm2(W[c]);
+    } else if (p == 0) {
+#pragma unroll
+        for (int c = 0; c < 5; ++c) m.w[c].warm3(W[c]);
+    } else {
+#pragma unroll
+        for (int c = 0; c < 5; ++c) m.w[c].push(W[c]);
+        if (p >= 2) {
+            // face f = p-2 between zones p-3 and p-2
+            double WL[5], WR[5], F[5];
+#pragma unroll
+            for (int c = 0; c < 5; ++c) { WL[c] = m.w[c].qpL; WR[c] = m.w[c].qm; }
+            WL[0] = dmax(WL[0], g.small_dens); WR[0] = dmax(WR[0], g.small_dens);
+            WL[4] = dmax(WL[4], g.small_pres); WR[4] = dmax(WR[4], g.small_pres);
+            hllc<D>(g, WL, WR, F);
+            fm_slot[(p - 2) * NTHR] = F[0];
+            if (p >= 3) {
+                const int q = p - 3;                     // zone of the pencil that is now complete
+                const int sp = (D == 0) ? (b * TILE + a) * PART_PITCH + q
+                             : (D == 1) ? (b * TILE + q) * PART_PITCH + a
+                                        : (q * TILE + b) * PART_PITCH + a;
+                if (D == 0) {
+#pragma unroll
+                    for (int c = 0; c < 5; ++c) part[c * PART_COMP + sp] = (F[c] - m.Fprev[c]) * nrd;
+                } else if (D == 1) {
+#pragma unroll
+                    for (int c = 0; c < 5; ++c)
+                        part[c * PART_COMP + sp] = fma(F[c] - m.Fprev[c], nrd, part[c * PART_COMP + sp]);
+                } else {
+                    double A5[5];
+#pragma unroll
+                    for (int c = 0; c < 5; ++c) A5[c] = fma(F[c] - m.Fprev[c], nrd, part[c * PART_COMP + sp]);
+                    const long long zc = z0 + (long long)q * stride;
+                    const bool grav = (g.grav[0] != 0.0) || (g.grav[1] != 0.0) || (g.grav[2] != 0.0);
+                    double Um[5];
+                    if (grav || NR >= 0) {
+#pragma unroll
+                        for (int c = 0; c < 5; ++c) Um[c] = Ub[c * g.comp_g + zc];
+                    }
+                    if (grav) {     // S4 source: constant gravity from the zone-centre state
+                        A5[1] = fma(Um[0], g.grav[0], A5[1]);
+                        A5[2] = fma(Um[0], g.grav[1], A5[2]);
+                        A5[3] = fma(Um[0], g.grav[2], A5[3]);
+                        A5[4] += fma(Um[3], g.grav[2], fma(Um[2], g.grav[1], Um[1] * g.grav[0]));
+                    }
+                    const long long ia0 = (long long)tc.b * g.box_a +
+                        ((long long)(tc.k0 + q) * g.ny + (tc.j0 + b)) * g.nx + (tc.i0 + a);
+#pragma unroll
+                    for (int c = 0; c < 5; ++c) {
+                        const long long ia = ia0 + c * g.comp_a;
+                        if (NR >= 0)
+                            up.U_next[(long long)tc.b * g.box_g + c * g.comp_g + zc] =
+                                node_update<NR>(up, Um[c], A5[c], ia);
+                        A[ia] = A5[c];
+                    }
+                }
+            }
+#pragma unroll
+            for (int c = 0; c < 5; ++c) m.Fprev[c] = F[c];
+        }
+    }
+}
+
+template <int D, int NR>
+__device__ __forceinline__ void hydro_sweep_full(const Geom& g, const TileCoord& tc, const double* __restrict__ Ub,
+                                                 double* __restrict__ part, double* __restrict__ fm_tile,
+                                                 double* __restrict__ rinv_b, double* __restrict__ A,
+                                                 const UpdArgs& up)
+{
+    const int ng = CST_NG;
+    constexpr int L = TILE;
+    const int tid = threadIdx.x, a = tid & (TILE - 1), b = tid >> 4;
+    long long z0, stride;
+    int n_d, o_d;
+    if (D == 0) {
+        z0 = ((long long)(tc.k0 + b + ng) * g.ey + (tc.j0 + a + ng)) * g.ex + (tc.i0 + ng);
+        stride = 1; n_d = g.nx; o_d = tc.i0;
+    } else if (D == 1) {
+        z0 = ((long long)(tc.k0 + b + ng) * g.ey + (tc.j0 + ng)) * g.ex + (tc.i0 + a + ng);
+        stride = g.ex; n_d = g.ny; o_d = tc.j0;
+    } else {
+        z0 = ((long long)(tc.k0 + ng) * g.ey + (tc.j0 + b + ng)) * g.ex + (tc.i0 + a + ng);
+        stride = g.plane_g; n_d = g.nz; o_d = tc.k0;
+    }
+    const bool ghost_lo = (o_d == 0), ghost_hi = (o_d + L == n_d);
+    double* fm_slot = fm_tile + (D * (TILE + 1)) * NTHR + tid;
+    HydroMarch m;
+
+    if (D == 0) {
+        // groups of four zones p = 4G .. 4G+3, G = -1 .. 4; zone p = -4 and p = 19 are not used
+        double cur[5][4], nxt[5][4];
+#pragma unroll
+        for (int c = 0; c < 5; ++c) ldg256(Ub + c * g.comp_g + z0 - 4, cur[c]);
+#pragma unroll
+        for (int G = -1; G <= 4; ++G) {
+            if (G < 4) {
+#pragma unroll
+                for (int c = 0; c < 5; ++c) ldg256(Ub + c * g.comp_g + z0 + 4 * (G + 1), nxt[c]);
+            }
+#pragma unroll
+            for (int e = 0; e < 4; ++e) {
+                const int p = 4 * G + e;
+                if (p >= -3 && p <= L + 2) {
+                    const double Uc[5] = { cur[0][e], cur[1][e], cur[2][e], cur[3][e], cur[4][e] };
+                    hydro_zone<D, NR>(g, tc, m, p, Uc, Ub, part, fm_slot, rinv_b, A, up, z0, stride, ghost_lo, ghost_hi, a, b);
+                }
+            }
+#pragma unroll
+            for (int c = 0; c < 5; ++c)
+#pragma unroll
+                for (int e = 0; e < 4; ++e) cur[c][e] = nxt[c][e];
+        }
+    } else {
+        double Uc[5], Un[5];
+#pragma unroll
+        for (int c = 0; c < 5; ++c) Uc[c] = Ub[c * g.comp_g + z0 - 3 * stride];
+#pragma unroll
+        for (int p = -3; p <= L + 2; ++p) {
+            if (p < L + 2) {
+                const long long zn = z0 + (long long)(p + 1) * stride;
+#pragma unroll
+                for (int c = 0; c < 5; ++c) Un[c] = Ub[c * g.comp_g + zn];
+            }
+            hydro_zone<D, NR>(g, tc, m, p, Uc, Ub, part, fm_slot, rinv_b, A, up, z0, stride, ghost_lo, ghost_hi, a, b);
+#pragma unroll
+            for (int c = 0; c < 5; ++c) Uc[c] = Un[c];
+        }
+    }
+}
+
+// --------------------------------------------------------------------------- any tile extent ----
+template <int D, int NR>
 __device__ __forceinline__ void hydro_sweep(const Geom& g, const TileCoord& tc, const double* __restrict__ Ub,
                                             double* __restrict__ part, double* __restrict__ fm_tile,
                                             double* __restrict__ rinv_b, double* __restrict__ A,
@@ -109,7 +279,7 @@ __device__ __forceinline__ void hydro_sweep(const Geom& g, const TileCoord& tc, 
                         const long long zc = z0 + (long long)q * stride;
                         const bool grav = (g.grav[0] != 0.0) || (g.grav[1] != 0.0) || (g.grav[2] != 0.0);
                         double Um[5];
-                        if (grav || up.fused) {
+                        if (grav || NR >= 0) {
 #pragma unroll
                             for (int c = 0; c < 5; ++c) Um[c] = Ub[c * g.comp_g + zc];
                         }
@@ -124,9 +294,9 @@ __device__ __forceinline__ void hydro_sweep(const Geom& g, const TileCoord& tc, 
 #pragma unroll
                         for (int c = 0; c < 5; ++c) {
                             const long long ia = ia0 + c * g.comp_a;
-                            if (up.fused)
+                            if (NR >= 0)
                                 up.U_next[(long long)tc.b * g.box_g + c * g.comp_g + zc] =
-                                    node_update(up, Um[c], A5[c], ia);
+                                    node_update<NR>(up, Um[c], A5[c], ia);
                             A[ia] = A5[c];
                         }
                     }
@@ -140,36 +310,61 @@ __device__ __forceinline__ void hydro_sweep(const Geom& g, const TileCoord& tc, 
     }
 }
 
+template <int NR>
 __global__ void __launch_bounds__(NTHR, 1)
 k_advect_hydro(Geom g, TileGeom tg, const double* __restrict__ U, double* __restrict__ A,
-               double* __restrict__ rinv, double* __restrict__ Fm, UpdArgs up)
+               double* __restrict__ rinv, double* __restrict__ Fm, UpdArgs up, bool x_vec)
 {
     extern __shared__ double part[];                   // [5][TILE][TILE][PART_PITCH]
     const TileCoord tc = tile_coord(g, tg, blockIdx.x);
     const double* Ub = U + (long long)tc.b * g.box_g;
     double* rinv_b = rinv + (long long)tc.b * g.comp_g;
     double* fm_tile = Fm + tc.tile * 3LL * (TILE + 1) * NTHR;
-    hydro_sweep<0>(g, tc, Ub, part, fm_tile, rinv_b, A, up);
-    __syncthreads();
-    hydro_sweep<1>(g, tc, Ub, part, fm_tile, rinv_b, A, up);
-    __syncthreads();
-    hydro_sweep<2>(g, tc, Ub, part, fm_tile, rinv_b, A, up);
+    const bool full = (tc.tx == TILE) && (tc.ty == TILE) && (tc.tz == TILE) && x_vec;
+    if (full) {
+        hydro_sweep_full<0, NR>(g, tc, Ub, part, fm_tile, rinv_b, A, up);
+        __syncthreads();
+        hydro_sweep_full<1, NR>(g, tc, Ub, part, fm_tile, rinv_b, A, up);
+        __syncthreads();
+        hydro_sweep_full<2, NR>(g, tc, Ub, part, fm_tile, rinv_b, A, up);
+    } else {
+        hydro_sweep<0, NR>(g, tc, Ub, part, fm_tile, rinv_b, A, up);
+        __syncthreads();
+        hydro_sweep<1, NR>(g, tc, Ub, part, fm_tile, rinv_b, A, up);
+        __syncthreads();
+        hydro_sweep<2, NR>(g, tc, Ub, part, fm_tile, rinv_b, A, up);
+    }
 }
 
-int launch_advect_hydro(cst_ctx* ctx, const double* U, double* A, const UpdArgs& up, cudaStream_t st)
+template <int NR>
+static int launch_hydro_nr(cst_ctx* ctx, const double* U, double* A, const UpdArgs& up, cudaStream_t st)
 {
     const Geom& g = ctx->g;
     const TileGeom tg = make_tile_geom(g);
     const size_t smem = 5ull * PART_COMP * sizeof(double);
     static bool attr_set = false;
     if (!attr_set) {
-        if (cudaFuncSetAttribute(k_advect_hydro, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
+        if (cudaFuncSetAttribute(k_advect_hydro<NR>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
             return CST_ECUDA;
         attr_set = true;
     }
     double* rinv = ctx->ws;
     double* Fm = ctx->ws + ws_rinv_doubles(g);
-    k_advect_hydro<<<(unsigned)tg.ntiles, NTHR, smem, st>>>(g, tg, U, A, rinv, Fm, up);
+    // 32-byte loads of the x sweep need rows that start on 32-byte boundaries
+    const bool x_vec = (g.nx % 4 == 0) && (((uintptr_t)U & 31) == 0);
+    k_advect_hydro<NR><<<(unsigned)tg.ntiles, NTHR, smem, st>>>(g, tg, U, A, rinv, Fm, up, x_vec);
     ctx->launches++;
     return cudaGetLastError() == cudaSuccess ? CST_OK : CST_ECUDA;
+}
+
+int launch_advect_hydro(cst_ctx* ctx, const double* U, double* A, const UpdArgs& up, cudaStream_t st)
+{
+    switch (up.nr) {
+    case -1: return launch_hydro_nr<-1>(ctx, U, A, up, st);
+    case 0: return launch_hydro_nr<0>(ctx, U, A, up, st);
+    case 1: return launch_hydro_nr<1>(ctx, U, A, up, st);
+    case 2: return launch_hydro_nr<2>(ctx, U, A, up, st);
+    case 3: return launch_hydro_nr<3>(ctx, U, A, up, st);
+    }
+    return CST_EINVAL;
 }

@@ -60,23 +60,27 @@ __device__ __forceinline__ TileCoord tile_coord(const Geom& g, const TileGeom& t
     return t;
 }
 
-struct UpdArgs {              // the SDC node update fused behind A (S5); see include/cst.h
-    bool fused;
+#define UPD_MAX_EXT 3        // external arrays the fused update can read (more -> unfused calls)
+
+// The SDC node update fused behind A (S5, Eq. (2) of the paper with R = 0):
+//   U_next = U_m + dt_m (A_new - A_old) + sum_q w_q A_q
+// normalised on the host into  U_next = U_m + ca * A_new + sum_{r < nr} c[r] * P[r]
+// where every occurrence of the A_new buffer among A_old / A_q is folded into ca and equal
+// pointers are merged (advect.cu make_upd).  nr = -1: no update (plain cst_advance_A).
+struct UpdArgs {
+    int nr;
+    const double* U_m;        // the state A is evaluated on (ghosted layout)
     double* U_next;
-    double dt_m;
-    const double* A_old;      // nullptr = "the value just computed"
-    int nquad;
-    const double* Aq[CST_MAX_QUAD];   // nullptr = "the value just computed"
-    double w[CST_MAX_QUAD];
+    double ca;
+    const double* P[UPD_MAX_EXT];
+    double c[UPD_MAX_EXT];
 };
 
-// U_next = U_m + dt_m (A_new - A_old) + sum_q w_q A_q   (Eq. (2) of the paper, R = 0)
+template <int NR>
 __device__ __forceinline__ double node_update(const UpdArgs& up, double um, double a, long long ia)
 {
-    const double aold = up.A_old ? up.A_old[ia] : a;
-    double acc = 0.0;
+    double acc = fma(up.ca, a, um);
 #pragma unroll
-    for (int q = 0; q < CST_MAX_QUAD; ++q)
-        if (q < up.nquad) acc = fma(up.w[q], up.Aq[q] ? up.Aq[q][ia] : a, acc);
-    return fma(up.dt_m, a - aold, um) + acc;
+    for (int r = 0; r < NR; ++r) acc = fma(up.c[r], up.P[r][ia], acc);
+    return acc;
 }
