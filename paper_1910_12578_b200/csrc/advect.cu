@@ -16,7 +16,7 @@ long long workspace_bytes(const Geom& g)
 static bool make_upd(UpdArgs& up, const double* U, double* A, double* U_next, double dt_m,
                      const double* A_old_m, const QuadArgs& q)
 {
-    up.nr = 0; up.U_m = U; up.U_next = U_next; up.ca = 0.0;
+    up.nr = 0; up.U_m = U; up.U_next = U_next; up.ca = 0.0; up.A_base = A;
     for (int r = 0; r < UPD_MAX_EXT; ++r) { up.P[r] = nullptr; up.c[r] = 0.0; }
     auto add = [&](const double* ptr, double coef) -> bool {
         if (ptr == A) { up.ca += coef; return true; }
@@ -35,7 +35,7 @@ int launch_advance_A(cst_ctx* ctx, const double* U, double* A, double* U_next, d
 {
     if (!ctx->ws || ctx->ws_bytes < workspace_bytes(ctx->g)) return CST_ENOWORKSPACE;
     UpdArgs up{};
-    up.nr = -1; up.U_m = U;
+    up.nr = -1; up.U_m = U; up.A_base = A;
     bool split = false;
     if (fused && !make_upd(up, U, A, U_next, dt_m, A_old_m, q)) { up.nr = -1; split = true; }
     int rc = launch_advect_hydro(ctx, U, A, up, st);

@@ -21,6 +21,11 @@
 #define PART_COMP (TILE * TILE * PART_PITCH)           // doubles per component
 
 // ------------------------------------------------------------------------ full 16^3 tiles ----
+// The march is a short loop (x: 6 groups of 4 zones, y/z: 11 pairs of zones) so that its body stays
+// in the instruction cache.  Every zone runs the SAME window step (PpmWindow::push) from the first
+// halo zone on: a window that starts from zeros holds garbage for three steps, but the first
+// quantities that are used (the parabola of zone -1, from p = 1) depend only on real zone values
+// (sweep.cuh), so no warm-up variants of the step are needed.
 __device__ __forceinline__ void ldg256(const double* p, double v[4])
 {   // one 32-byte sector per thread (p is 32-byte aligned)
     asm volatile("ld.global.nc.v4.f64 {%0,%1,%2,%3}, [%4];"
@@ -30,91 +35,89 @@ __device__ __forceinline__ void ldg256(const double* p, double v[4])
 struct HydroMarch {           // per-thread state of one pencil march
     PpmWindow w[5];
     double Fprev[5];
+    double* fm_slot;          // Fm slot of the face that completes next
+    double* part;             // shared-memory partial of the zone that completes next (component 0)
+    double* pA;               // z sweep: A of the zone that completes next (component 0)
+    long long zc;             // z sweep: ghosted index (within the box) of that zone
 };
 
-// one zone of the march: pencil position P (compile-time after unrolling), conserved state Uc
 template <int D, int NR>
 __device__ __forceinline__ void hydro_zone(const Geom& g, const TileCoord& tc, HydroMarch& m, const int p,
                                            const double Uc[5], const double* __restrict__ Ub,
-                                           double* __restrict__ part, double* __restrict__ fm_slot,
-                                           double* __restrict__ rinv_b, double* __restrict__ A, const UpdArgs& up,
+                                           double* __restrict__ rinv_b, const UpdArgs& up,
                                            const long long z0, const long long stride, const bool ghost_lo,
-                                           const bool ghost_hi, const int a, const int b)
+                                           const bool ghost_hi)
 {
     constexpr int L = TILE;
+    constexpr int PST = (D == 0) ? 1 : (D == 1) ? PART_PITCH : TILE * PART_PITCH;
     const double nrd = -((D == 0) ? g.rdx : (D == 1) ? g.rdy : g.rdz);
+    // z sweep: operands of the source term and of the fused node update of the zone that completes in
+    // this step are requested first, so that their latency hides behind the arithmetic below
+    const bool grav = (g.grav[0] != 0.0) || (g.grav[1] != 0.0) || (g.grav[2] != 0.0);
+    double Um[5], Pv[5][UPD_MAX_EXT];
+    long long ia0 = 0;
+    if (D == 2 && p >= 3) {
+        ia0 = m.pA - up.A_base;                          // index of component 0 in the A-like arrays
+        if (grav || NR >= 0) {
+#pragma unroll
+            for (int c = 0; c < 5; ++c) Um[c] = Ub[c * g.comp_g + m.zc];
+        }
+#pragma unroll
+        for (int c = 0; c < 5; ++c)
+#pragma unroll
+            for (int r = 0; r < NR; ++r) Pv[c][r] = up.P[r][ia0 + c * g.comp_a];
+    }
     double W[5];
     const double r = cons_to_prim(g, Uc[0], Uc[1], Uc[2], Uc[3], Uc[4], W);
     if ((D == 2 && p >= 0 && p < L) || (p < 0 && ghost_lo) || (p >= L && ghost_hi))
         rinv_b[z0 + (long long)p * stride] = r;
-    if (p == -3) {
 #pragma unroll
-        for (int c = 0; c < 5; ++c) m.w[c].start(W[c]);
-    } else if (p == -2) {
+    for (int c = 0; c < 5; ++c) m.w[c].push(W[c]);
+    if (p >= 2) {
+        // face f = p-2 between zones p-3 and p-2
+        double WL[5], WR[5], F[5];
 #pragma unroll
-        for (int c = 0; c < 5; ++c) m.w[c].warm1(W[c]);
-    } else if (p == -1) {
+        for (int c = 0; c < 5; ++c) { WL[c] = m.w[c].qpL; WR[c] = m.w[c].qm; }
+        WL[0] = dmax(WL[0], g.small_dens); WR[0] = dmax(WR[0], g.small_dens);
+        WL[4] = dmax(WL[4], g.small_pres); WR[4] = dmax(WR[4], g.small_pres);
+        hllc<D>(g, WL, WR, F);
+        *m.fm_slot = F[0];
+        m.fm_slot += NTHR;
+        if (p >= 3) {                                    // zone q = p-3 of the pencil is complete
+            if (D == 0) {
 #pragma unroll
-        for (int c = 0; c < 5; ++c) m.w[c].warm2(W[c]);
-    } else if (p == 0) {
+                for (int c = 0; c < 5; ++c) m.part[c * PART_COMP] = (F[c] - m.Fprev[c]) * nrd;
+            } else if (D == 1) {
 #pragma unroll
-        for (int c = 0; c < 5; ++c) m.w[c].warm3(W[c]);
-    } else {
+                for (int c = 0; c < 5; ++c)
+                    m.part[c * PART_COMP] = fma(F[c] - m.Fprev[c], nrd, m.part[c * PART_COMP]);
+            } else {
+                double A5[5];
 #pragma unroll
-        for (int c = 0; c < 5; ++c) m.w[c].push(W[c]);
-        if (p >= 2) {
-            // face f = p-2 between zones p-3 and p-2
-            double WL[5], WR[5], F[5];
-#pragma unroll
-            for (int c = 0; c < 5; ++c) { WL[c] = m.w[c].qpL; WR[c] = m.w[c].qm; }
-            WL[0] = dmax(WL[0], g.small_dens); WR[0] = dmax(WR[0], g.small_dens);
-            WL[4] = dmax(WL[4], g.small_pres); WR[4] = dmax(WR[4], g.small_pres);
-            hllc<D>(g, WL, WR, F);
-            fm_slot[(p - 2) * NTHR] = F[0];
-            if (p >= 3) {
-                const int q = p - 3;                     // zone of the pencil that is now complete
-                const int sp = (D == 0) ? (b * TILE + a) * PART_PITCH + q
-                             : (D == 1) ? (b * TILE + q) * PART_PITCH + a
-                                        : (q * TILE + b) * PART_PITCH + a;
-                if (D == 0) {
-#pragma unroll
-                    for (int c = 0; c < 5; ++c) part[c * PART_COMP + sp] = (F[c] - m.Fprev[c]) * nrd;
-                } else if (D == 1) {
-#pragma unroll
-                    for (int c = 0; c < 5; ++c)
-                        part[c * PART_COMP + sp] = fma(F[c] - m.Fprev[c], nrd, part[c * PART_COMP + sp]);
-                } else {
-                    double A5[5];
-#pragma unroll
-                    for (int c = 0; c < 5; ++c) A5[c] = fma(F[c] - m.Fprev[c], nrd, part[c * PART_COMP + sp]);
-                    const long long zc = z0 + (long long)q * stride;
-                    const bool grav = (g.grav[0] != 0.0) || (g.grav[1] != 0.0) || (g.grav[2] != 0.0);
-                    double Um[5];
-                    if (grav || NR >= 0) {
-#pragma unroll
-                        for (int c = 0; c < 5; ++c) Um[c] = Ub[c * g.comp_g + zc];
-                    }
-                    if (grav) {     // S4 source: constant gravity from the zone-centre state
-                        A5[1] = fma(Um[0], g.grav[0], A5[1]);
-                        A5[2] = fma(Um[0], g.grav[1], A5[2]);
-                        A5[3] = fma(Um[0], g.grav[2], A5[3]);
-                        A5[4] += fma(Um[3], g.grav[2], fma(Um[2], g.grav[1], Um[1] * g.grav[0]));
-                    }
-                    const long long ia0 = (long long)tc.b * g.box_a +
-                        ((long long)(tc.k0 + q) * g.ny + (tc.j0 + b)) * g.nx + (tc.i0 + a);
-#pragma unroll
-                    for (int c = 0; c < 5; ++c) {
-                        const long long ia = ia0 + c * g.comp_a;
-                        if (NR >= 0)
-                            up.U_next[(long long)tc.b * g.box_g + c * g.comp_g + zc] =
-                                node_update<NR>(up, Um[c], A5[c], ia);
-                        A[ia] = A5[c];
-                    }
+                for (int c = 0; c < 5; ++c) A5[c] = fma(F[c] - m.Fprev[c], nrd, m.part[c * PART_COMP]);
+                if (grav) {     // S4 source: constant gravity from the zone-centre state
+                    A5[1] = fma(Um[0], g.grav[0], A5[1]);
+                    A5[2] = fma(Um[0], g.grav[1], A5[2]);
+                    A5[3] = fma(Um[0], g.grav[2], A5[3]);
+                    A5[4] += fma(Um[3], g.grav[2], fma(Um[2], g.grav[1], Um[1] * g.grav[0]));
                 }
-            }
 #pragma unroll
-            for (int c = 0; c < 5; ++c) m.Fprev[c] = F[c];
+                for (int c = 0; c < 5; ++c) {
+                    if (NR >= 0) {
+                        double acc = fma(up.ca, A5[c], Um[c]);
+#pragma unroll
+                        for (int r = 0; r < NR; ++r) acc = fma(up.c[r], Pv[c][r], acc);
+                        up.U_next[(long long)tc.b * g.box_g + c * g.comp_g + m.zc] = acc;
+                    }
+                    m.pA[c * g.comp_a] = A5[c];
+                }
+                m.pA += (long long)g.ny * g.nx;
+                m.zc += stride;
+            }
+            m.part += PST;
         }
+#pragma unroll
+        for (int c = 0; c < 5; ++c) m.Fprev[c] = F[c];
     }
 }
 
@@ -128,27 +131,35 @@ __device__ __forceinline__ void hydro_sweep_full(const Geom& g, const TileCoord&
     constexpr int L = TILE;
     const int tid = threadIdx.x, a = tid & (TILE - 1), b = tid >> 4;
     long long z0, stride;
-    int n_d, o_d;
+    int n_d, o_d, sp0;
     if (D == 0) {
         z0 = ((long long)(tc.k0 + b + ng) * g.ey + (tc.j0 + a + ng)) * g.ex + (tc.i0 + ng);
-        stride = 1; n_d = g.nx; o_d = tc.i0;
+        stride = 1; n_d = g.nx; o_d = tc.i0; sp0 = (b * TILE + a) * PART_PITCH;
     } else if (D == 1) {
         z0 = ((long long)(tc.k0 + b + ng) * g.ey + (tc.j0 + ng)) * g.ex + (tc.i0 + a + ng);
-        stride = g.ex; n_d = g.ny; o_d = tc.j0;
+        stride = g.ex; n_d = g.ny; o_d = tc.j0; sp0 = (b * TILE) * PART_PITCH + a;
     } else {
         z0 = ((long long)(tc.k0 + ng) * g.ey + (tc.j0 + b + ng)) * g.ex + (tc.i0 + a + ng);
-        stride = g.plane_g; n_d = g.nz; o_d = tc.k0;
+        stride = g.plane_g; n_d = g.nz; o_d = tc.k0; sp0 = b * PART_PITCH + a;
     }
     const bool ghost_lo = (o_d == 0), ghost_hi = (o_d + L == n_d);
-    double* fm_slot = fm_tile + (D * (TILE + 1)) * NTHR + tid;
     HydroMarch m;
+#pragma unroll
+    for (int c = 0; c < 5; ++c) {
+        m.w[c].q1 = m.w[c].q2 = m.w[c].dq1 = m.w[c].s2 = m.w[c].e = m.w[c].qp = 0.0;
+        m.Fprev[c] = 0.0;
+    }
+    m.fm_slot = fm_tile + (D * (TILE + 1)) * NTHR + tid;
+    m.part = part + sp0;
+    m.pA = A + (long long)tc.b * g.box_a + ((long long)tc.k0 * g.ny + (tc.j0 + b)) * g.nx + (tc.i0 + a);
+    m.zc = z0;
 
     if (D == 0) {
-        // groups of four zones p = 4G .. 4G+3, G = -1 .. 4; zone p = -4 and p = 19 are not used
+        // groups of four zones p = 4G .. 4G+3, G = -1 .. 4; zones p = -4 and p = 19 are not used
         double cur[5][4], nxt[5][4];
 #pragma unroll
         for (int c = 0; c < 5; ++c) ldg256(Ub + c * g.comp_g + z0 - 4, cur[c]);
-#pragma unroll
+#pragma unroll 1
         for (int G = -1; G <= 4; ++G) {
             if (G < 4) {
 #pragma unroll
@@ -157,10 +168,9 @@ __device__ __forceinline__ void hydro_sweep_full(const Geom& g, const TileCoord&
 #pragma unroll
             for (int e = 0; e < 4; ++e) {
                 const int p = 4 * G + e;
-                if (p >= -3 && p <= L + 2) {
-                    const double Uc[5] = { cur[0][e], cur[1][e], cur[2][e], cur[3][e], cur[4][e] };
-                    hydro_zone<D, NR>(g, tc, m, p, Uc, Ub, part, fm_slot, rinv_b, A, up, z0, stride, ghost_lo, ghost_hi, a, b);
-                }
+                if ((e == 0 && G == -1) || (e == 3 && G == 4)) continue;
+                const double Uc[5] = { cur[0][e], cur[1][e], cur[2][e], cur[3][e], cur[4][e] };
+                hydro_zone<D, NR>(g, tc, m, p, Uc, Ub, rinv_b, up, z0, stride, ghost_lo, ghost_hi);
             }
 #pragma unroll
             for (int c = 0; c < 5; ++c)
@@ -168,19 +178,30 @@ __device__ __forceinline__ void hydro_sweep_full(const Geom& g, const TileCoord&
                 for (int e = 0; e < 4; ++e) cur[c][e] = nxt[c][e];
         }
     } else {
-        double Uc[5], Un[5];
+        // pairs of zones p = -3 + 2n, -2 + 2n, n = 0 .. 10, loaded one pair ahead
+        double cur[5][2], nxt[5][2];
 #pragma unroll
-        for (int c = 0; c < 5; ++c) Uc[c] = Ub[c * g.comp_g + z0 - 3 * stride];
+        for (int c = 0; c < 5; ++c)
 #pragma unroll
-        for (int p = -3; p <= L + 2; ++p) {
-            if (p < L + 2) {
-                const long long zn = z0 + (long long)(p + 1) * stride;
+            for (int e = 0; e < 2; ++e) cur[c][e] = Ub[c * g.comp_g + z0 + (e - 3) * stride];
+#pragma unroll 1
+        for (int n = 0; n <= 10; ++n) {
+            const int p0 = 2 * n - 3;
+            if (n < 10) {
 #pragma unroll
-                for (int c = 0; c < 5; ++c) Un[c] = Ub[c * g.comp_g + zn];
+                for (int c = 0; c < 5; ++c)
+#pragma unroll
+                    for (int e = 0; e < 2; ++e) nxt[c][e] = Ub[c * g.comp_g + z0 + (long long)(p0 + 2 + e) * stride];
             }
-            hydro_zone<D, NR>(g, tc, m, p, Uc, Ub, part, fm_slot, rinv_b, A, up, z0, stride, ghost_lo, ghost_hi, a, b);
 #pragma unroll
-            for (int c = 0; c < 5; ++c) Uc[c] = Un[c];
+            for (int e = 0; e < 2; ++e) {
+                const double Uc[5] = { cur[0][e], cur[1][e], cur[2][e], cur[3][e], cur[4][e] };
+                hydro_zone<D, NR>(g, tc, m, p0 + e, Uc, Ub, rinv_b, up, z0, stride, ghost_lo, ghost_hi);
+            }
+#pragma unroll
+            for (int c = 0; c < 5; ++c)
+#pragma unroll
+                for (int e = 0; e < 2; ++e) cur[c][e] = nxt[c][e];
         }
     }
 }

@@ -14,7 +14,7 @@
 //   species_sweep_full  -- the tile is a full 16^3: the march is unrolled at compile time (the
 //                          window slides by register renaming, shared-memory offsets are immediates);
 //   species_sweep       -- any tile extent (ragged edges of boxes whose sides are not multiples of 16).
-// Shared memory: 2 x 16*16*17 doubles = 69.6 KB per CTA, so three CTAs (24 warps) share an SM.
+// Shared memory: 2 x 16*16*17 + 18*256 doubles = 106.5 KB per CTA, so two CTAs (16 warps) share an SM.
 #include "sweep.cuh"
 #include "tile.cuh"
 
@@ -22,65 +22,46 @@
 #define SP_TILE (TILE * TILE * SP_PITCH)
 
 // ------------------------------------------------------------------------ full 16^3 tiles ----
-template <int D, int NR>
-__device__ __forceinline__ void species_sweep_full(const Geom& g, const TileCoord& tc, const double* __restrict__ Us,
-                                                   const double* __restrict__ rinv_b,
-                                                   const double* __restrict__ Xs, double* __restrict__ Ps,
-                                                   const double* __restrict__ fm_tile,
-                                                   double* __restrict__ A, int c, const UpdArgs& up)
+// Shared memory of the fast path: Xs (core of X), Ps (A under construction), Hs (halo X values,
+// [direction][n = 0..5][tid]: n < 3 are pencil positions -3..-1, n >= 3 are 16..18, stored under the
+// thread id of the pencil that reads them).  All global->shared traffic of a species happens in
+// one streaming phase with many independent loads in flight; the sweeps touch global memory only
+// for the face mass fluxes, which are loaded one sweep ahead into registers.
+#define SP_HALO (3 * 6 * NTHR)
+
+struct PencilGeom {           // per-thread constants of the three pencils
+    long long z0[3];          // ghosted index (within a component of the box) of pencil position 0
+    long long stride[3];
+};
+
+__device__ __forceinline__ void load_fm(const double* __restrict__ fm_tile, int D, double fmv[TILE + 1])
 {
-    const int ng = CST_NG;
+    const double* __restrict__ fm = fm_tile + (D * (TILE + 1)) * NTHR + threadIdx.x;
+#pragma unroll
+    for (int f = 0; f <= TILE; ++f) fmv[f] = fm[f * NTHR];
+}
+
+template <int D>
+__device__ __forceinline__ void species_sweep_full(const Geom& g, const double* __restrict__ Xs,
+                                                   double* __restrict__ Ps, const double* __restrict__ Hs,
+                                                   const double fmv[TILE + 1])
+{
     const int tid = threadIdx.x, a = tid & (TILE - 1), b = tid >> 4;
     constexpr int L = TILE;
     constexpr int SST = (D == 0) ? 1 : (D == 1) ? SP_PITCH : TILE * SP_PITCH;   // smem stride along the pencil
-    long long z0, stride;
-    int s0;
-    if (D == 0) {
-        z0 = ((long long)(tc.k0 + b + ng) * g.ey + (tc.j0 + a + ng)) * g.ex + (tc.i0 + ng);
-        stride = 1; s0 = (b * TILE + a) * SP_PITCH;
-    } else if (D == 1) {
-        z0 = ((long long)(tc.k0 + b + ng) * g.ey + (tc.j0 + ng)) * g.ex + (tc.i0 + a + ng);
-        stride = g.ex; s0 = (b * TILE) * SP_PITCH + a;
-    } else {
-        z0 = ((long long)(tc.k0 + ng) * g.ey + (tc.j0 + b + ng)) * g.ex + (tc.i0 + a + ng);
-        stride = g.plane_g; s0 = b * SP_PITCH + a;
-    }
+    const int s0 = (D == 0) ? (b * TILE + a) * SP_PITCH : (D == 1) ? (b * TILE) * SP_PITCH + a : b * SP_PITCH + a;
     const double nrd = -((D == 0) ? g.rdx : (D == 1) ? g.rdy : g.rdz);
-    const double* __restrict__ fm = fm_tile + (D * (TILE + 1)) * NTHR + tid;
     const double* __restrict__ xs = Xs + s0;
     double* __restrict__ ps = Ps + s0;
-
-    // halo zones p = -3..-1 and L..L+2 from global memory
-    double hlo[3], hhi[3];
-#pragma unroll
-    for (int n = 0; n < 3; ++n) {
-        const long long zl = z0 + (long long)(n - 3) * stride, zh = z0 + (long long)(L + n) * stride;
-        hlo[n] = Us[zl] * rinv_b[zl];
-        hhi[n] = Us[zh] * rinv_b[zh];
-    }
-    // face mass fluxes of the pencil (thread-private slots, coalesced)
-    double fmv[L + 1];
-#pragma unroll
-    for (int f = 0; f <= L; ++f) fmv[f] = fm[f * NTHR];
+    const double* __restrict__ hs = Hs + D * 6 * NTHR + tid;
 
     PpmWindow w;
-    w.start(hlo[0]); w.warm1(hlo[1]); w.warm2(hlo[2]);
+    w.start(hs[0]); w.warm1(hs[NTHR]); w.warm2(hs[2 * NTHR]);
     w.warm3(xs[0]);
     double Fprev = 0.0;
-    // output addressing of the z sweep (D == 2): running pointers to zone q of the pencil
-    const long long ia0 = (long long)tc.b * g.box_a + (long long)c * g.comp_a +
-        ((long long)tc.k0 * g.ny + (tc.j0 + b)) * g.nx + (tc.i0 + a);
-    const long long plane_a = (long long)g.ny * g.nx;
-    const long long iu0 = (long long)tc.b * g.box_g + (long long)c * g.comp_g + z0;
-    double* pA = A + ia0;
-    const double* pU = up.U_m + iu0;
-    double* pUn = up.U_next + iu0;
-    const double* pP[UPD_MAX_EXT];
-#pragma unroll
-    for (int r = 0; r < UPD_MAX_EXT; ++r) pP[r] = (r < NR) ? up.P[r] + ia0 : nullptr;
 #pragma unroll
     for (int p = 1; p <= L + 2; ++p) {
-        const double qn = (p < L) ? xs[p * SST] : hhi[p - L];
+        const double qn = (p < L) ? xs[p * SST] : hs[(3 + p - L) * NTHR];
         w.push(qn);
         if (p >= 2) {
             const double fmc = fmv[p - 2];              // mass flux of face f = p-2
@@ -89,22 +70,110 @@ __device__ __forceinline__ void species_sweep_full(const Geom& g, const TileCoor
                 const int q = p - 3;
                 const double dF = F - Fprev;
                 if (D == 0) ps[q * SST] = dF * nrd;
-                else if (D == 1) ps[q * SST] = fma(dF, nrd, ps[q * SST]);
-                else {
-                    const double av = fma(dF, nrd, ps[q * SST]);
-                    if (NR >= 0) {
-                        double acc = fma(up.ca, av, *pU);
-#pragma unroll
-                        for (int r = 0; r < NR; ++r) { acc = fma(up.c[r], *pP[r], acc); pP[r] += plane_a; }
-                        *pUn = acc;
-                        pU += stride; pUn += stride;
-                    }
-                    *pA = av;
-                    pA += plane_a;
-                }
+                else ps[q * SST] = fma(dF, nrd, ps[q * SST]);
             }
             Fprev = F;
         }
+    }
+}
+
+// streaming phase: write out species c_out (A and, fused, U_next) from Ps, stage species c_in into Xs / Hs
+template <int NR>
+__device__ __forceinline__ void species_stream_full(const Geom& g, const TileCoord& tc, const PencilGeom& pg,
+                                                    const double* __restrict__ Ub, const double* __restrict__ rinv_b,
+                                                    double* __restrict__ Xs, const double* __restrict__ Ps,
+                                                    double* __restrict__ Hs, double* __restrict__ A,
+                                                    const UpdArgs& up, const int c_out, const int c_in)
+{
+    const int ng = CST_NG;
+    const int tid = threadIdx.x, ti = tid & (TILE - 1), tr = tid >> 4;
+    // ghosted index of the tile zone (i = ti, j = tr, k = 0); row n of this thread is k = n
+    const long long zt = ((long long)(tc.k0 + ng) * g.ey + (tc.j0 + tr + ng)) * g.ex + (tc.i0 + ti + ng);
+    if (c_in >= 0) {
+        const double* __restrict__ Us = Ub + (long long)c_in * g.comp_g;
+#pragma unroll
+        for (int k = 0; k < TILE; ++k) {
+            const long long z = zt + k * g.plane_g;
+            Xs[(k * TILE + tr) * SP_PITCH + ti] = Us[z] * rinv_b[z];
+        }
+#pragma unroll
+        for (int d = 0; d < 3; ++d)
+#pragma unroll
+            for (int n = 0; n < 6; ++n) {
+                const long long z = pg.z0[d] + (long long)(n < 3 ? n - 3 : TILE - 3 + n) * pg.stride[d];
+                Hs[(d * 6 + n) * NTHR + tid] = Us[z] * rinv_b[z];
+            }
+    }
+    if (c_out >= 0) {
+        const long long plane_a = (long long)g.ny * g.nx;
+        const long long ia0 = (long long)tc.b * g.box_a + (long long)c_out * g.comp_a +
+            ((long long)tc.k0 * g.ny + (tc.j0 + tr)) * g.nx + (tc.i0 + ti);
+        const long long iu0 = (long long)tc.b * g.box_g + (long long)c_out * g.comp_g + zt;
+        // batches of four zones: every load of a batch is issued before its first store (the
+        // compiler may not move loads over stores that could alias them)
+#pragma unroll
+        for (int k0 = 0; k0 < TILE; k0 += 4) {
+            double av[4], um[4], pv[4][UPD_MAX_EXT];
+#pragma unroll
+            for (int e = 0; e < 4; ++e) {
+                const int k = k0 + e;
+                av[e] = Ps[(k * TILE + tr) * SP_PITCH + ti];
+                if (NR >= 0) {
+                    um[e] = up.U_m[iu0 + k * g.plane_g];
+#pragma unroll
+                    for (int r = 0; r < NR; ++r) pv[e][r] = up.P[r][ia0 + k * plane_a];
+                }
+            }
+#pragma unroll
+            for (int e = 0; e < 4; ++e) {
+                const int k = k0 + e;
+                if (NR >= 0) {
+                    double acc = fma(up.ca, av[e], um[e]);
+#pragma unroll
+                    for (int r = 0; r < NR; ++r) acc = fma(up.c[r], pv[e][r], acc);
+                    up.U_next[iu0 + k * g.plane_g] = acc;
+                }
+                A[ia0 + k * plane_a] = av[e];
+            }
+        }
+    }
+}
+
+template <int NR>
+__device__ __forceinline__ void species_tile_full(const Geom& g, const TileCoord& tc, const double* __restrict__ Ub,
+                                                  const double* __restrict__ rinv_b,
+                                                  const double* __restrict__ fm_tile, double* __restrict__ A,
+                                                  const UpdArgs& up, double* __restrict__ sm)
+{
+    double* Xs = sm;
+    double* Ps = sm + SP_TILE;
+    double* Hs = sm + 2 * SP_TILE;
+    const int ng = CST_NG;
+    const int tid = threadIdx.x, a = tid & (TILE - 1), b = tid >> 4;
+    PencilGeom pg;
+    pg.z0[0] = ((long long)(tc.k0 + b + ng) * g.ey + (tc.j0 + a + ng)) * g.ex + (tc.i0 + ng);
+    pg.z0[1] = ((long long)(tc.k0 + b + ng) * g.ey + (tc.j0 + ng)) * g.ex + (tc.i0 + a + ng);
+    pg.z0[2] = ((long long)(tc.k0 + ng) * g.ey + (tc.j0 + b + ng)) * g.ex + (tc.i0 + a + ng);
+    pg.stride[0] = 1; pg.stride[1] = g.ex; pg.stride[2] = g.plane_g;
+
+    double fmc[TILE + 1], fmn[TILE + 1];
+    load_fm(fm_tile, 0, fmc);
+    for (int s = 0; s <= g.nspec; ++s) {
+        __syncthreads();                                // z sweep of species s-1 done; Xs, Hs free
+        species_stream_full<NR>(g, tc, pg, Ub, rinv_b, Xs, Ps, Hs, A, up,
+                                s > 0 ? 5 + s - 1 : -1, s < g.nspec ? 5 + s : -1);
+        if (s == g.nspec) break;
+        __syncthreads();
+        load_fm(fm_tile, 1, fmn);
+        species_sweep_full<0>(g, Xs, Ps, Hs, fmc);
+        __syncthreads();
+        load_fm(fm_tile, 2, fmc);
+        species_sweep_full<1>(g, Xs, Ps, Hs, fmn);
+        __syncthreads();
+        load_fm(fm_tile, 0, fmn);
+        species_sweep_full<2>(g, Xs, Ps, Hs, fmc);
+#pragma unroll
+        for (int f = 0; f <= TILE; ++f) fmc[f] = fmn[f];
     }
 }
 
@@ -183,7 +252,7 @@ __device__ __forceinline__ void species_sweep(const Geom& g, const TileCoord& tc
 }
 
 template <int NR>
-__global__ void __launch_bounds__(NTHR, 3)
+__global__ void __launch_bounds__(NTHR, 2)
 k_advect_species(Geom g, TileGeom tg, const double* __restrict__ U, double* __restrict__ A,
                  const double* __restrict__ rinv, const double* __restrict__ Fm, UpdArgs up)
 {
@@ -196,41 +265,27 @@ k_advect_species(Geom g, TileGeom tg, const double* __restrict__ U, double* __re
     const double* rinv_b = rinv + (long long)tc.b * g.comp_g;
     const double* fm_tile = Fm + tc.tile * 3LL * (TILE + 1) * NTHR;
     const int tid = threadIdx.x, ti = tid & (TILE - 1), tr = tid >> 4;   // tr = row group 0..15
-    const bool full = (tc.tx == TILE) && (tc.ty == TILE) && (tc.tz == TILE);
-
+    if ((tc.tx == TILE) && (tc.ty == TILE) && (tc.tz == TILE)) {
+        species_tile_full<NR>(g, tc, Ub, rinv_b, fm_tile, A, up, sm);
+        return;
+    }
     // ghosted index of the tile zone (i = ti, j = tr, k = 0); row n of this thread is k = n
     const long long zt = ((long long)(tc.k0 + ng) * g.ey + (tc.j0 + tr + ng)) * g.ex + (tc.i0 + ti + ng);
     for (int s = 0; s < g.nspec; ++s) {
         const int c = 5 + s;
         const double* Us = Ub + (long long)c * g.comp_g;
         __syncthreads();                                // previous species done with Xs / Ps
-        if (full) {
-#pragma unroll
-            for (int k = 0; k < TILE; ++k) {
+        for (int k = 0; k < tc.tz; ++k)
+            if (tr < tc.ty && ti < tc.tx) {
                 const long long z = zt + k * g.plane_g;
                 Xs[(k * TILE + tr) * SP_PITCH + ti] = Us[z] * rinv_b[z];
             }
-        } else {
-            for (int k = 0; k < tc.tz; ++k)
-                if (tr < tc.ty && ti < tc.tx) {
-                    const long long z = zt + k * g.plane_g;
-                    Xs[(k * TILE + tr) * SP_PITCH + ti] = Us[z] * rinv_b[z];
-                }
-        }
         __syncthreads();
-        if (full) {
-            species_sweep_full<0, NR>(g, tc, Us, rinv_b, Xs, Ps, fm_tile, A, c, up);
-            __syncthreads();
-            species_sweep_full<1, NR>(g, tc, Us, rinv_b, Xs, Ps, fm_tile, A, c, up);
-            __syncthreads();
-            species_sweep_full<2, NR>(g, tc, Us, rinv_b, Xs, Ps, fm_tile, A, c, up);
-        } else {
-            species_sweep<0, NR>(g, tc, Us, rinv_b, Xs, Ps, fm_tile, A, c, up);
-            __syncthreads();
-            species_sweep<1, NR>(g, tc, Us, rinv_b, Xs, Ps, fm_tile, A, c, up);
-            __syncthreads();
-            species_sweep<2, NR>(g, tc, Us, rinv_b, Xs, Ps, fm_tile, A, c, up);
-        }
+        species_sweep<0, NR>(g, tc, Us, rinv_b, Xs, Ps, fm_tile, A, c, up);
+        __syncthreads();
+        species_sweep<1, NR>(g, tc, Us, rinv_b, Xs, Ps, fm_tile, A, c, up);
+        __syncthreads();
+        species_sweep<2, NR>(g, tc, Us, rinv_b, Xs, Ps, fm_tile, A, c, up);
     }
 }
 
@@ -239,7 +294,7 @@ static int launch_species_nr(cst_ctx* ctx, const double* U, double* A, const Upd
 {
     const Geom& g = ctx->g;
     const TileGeom tg = make_tile_geom(g);
-    const size_t smem = 2ull * SP_TILE * sizeof(double);
+    const size_t smem = (2ull * SP_TILE + SP_HALO) * sizeof(double);
     static bool attr_set = false;
     if (!attr_set) {
         if (cudaFuncSetAttribute(k_advect_species<NR>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)

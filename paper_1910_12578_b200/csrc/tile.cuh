@@ -71,6 +71,7 @@ struct UpdArgs {
     int nr;
     const double* U_m;        // the state A is evaluated on (ghosted layout)
     double* U_next;
+    const double* A_base;     // the A_new array (index origin of the A-like arrays)
     double ca;
     const double* P[UPD_MAX_EXT];
     double c[UPD_MAX_EXT];
