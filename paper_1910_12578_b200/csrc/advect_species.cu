@@ -29,16 +29,45 @@
 // for the face mass fluxes, which are loaded one sweep ahead into registers.
 #define SP_HALO (3 * 6 * NTHR)
 
-struct PencilGeom {           // per-thread constants of the three pencils
-    long long z0[3];          // ghosted index (within a component of the box) of pencil position 0
-    long long stride[3];
-};
+// L2 residency hints (PTX createpolicy / .L2::cache_hint): the face mass fluxes and 1/rho of a tile are
+// read again for each of the nspec species, so they should outlive the once-only streams (A_old
+// arrays in, A and U_next out) that pass through the same L2.
+__device__ __forceinline__ unsigned long long l2_policy_keep()
+{
+    unsigned long long p;
+    asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(p));
+    return p;
+}
+__device__ __forceinline__ unsigned long long l2_policy_stream()
+{
+    unsigned long long p;
+    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
+    return p;
+}
+__device__ __forceinline__ double ldg_hint(const double* a, unsigned long long pol)
+{
+    double v;
+    asm volatile("ld.global.nc.L2::cache_hint.f64 %0, [%1], %2;" : "=d"(v) : "l"(a), "l"(pol));
+    return v;
+}
+__device__ __forceinline__ double2 ldg2_hint(const double* a, unsigned long long pol)
+{
+    double2 v;
+    asm volatile("ld.global.nc.L2::cache_hint.v2.f64 {%0,%1}, [%2], %3;" : "=d"(v.x), "=d"(v.y) : "l"(a), "l"(pol));
+    return v;
+}
+__device__ __forceinline__ void stg2_hint(double* a, double2 v, unsigned long long pol)
+{
+    asm volatile("st.global.L2::cache_hint.v2.f64 [%0], {%1,%2}, %3;" :: "l"(a), "d"(v.x), "d"(v.y), "l"(pol) : "memory");
+}
+__device__ __forceinline__ double2 ldg2(const double* a) { return __ldg(reinterpret_cast<const double2*>(a)); }
 
 __device__ __forceinline__ void load_fm(const double* __restrict__ fm_tile, int D, double fmv[TILE + 1])
 {
+    const unsigned long long pol = l2_policy_keep();
     const double* __restrict__ fm = fm_tile + (D * (TILE + 1)) * NTHR + threadIdx.x;
 #pragma unroll
-    for (int f = 0; f <= TILE; ++f) fmv[f] = fm[f * NTHR];
+    for (int f = 0; f <= TILE; ++f) fmv[f] = ldg_hint(fm + f * NTHR, pol);
 }
 
 template <int D>
@@ -77,63 +106,89 @@ __device__ __forceinline__ void species_sweep_full(const Geom& g, const double* 
     }
 }
 
-// streaming phase: write out species c_out (A and, fused, U_next) from Ps, stage species c_in into Xs / Hs
+// streaming phase: write out species c_out (A and, fused, U_next) from Ps, stage species c_in into
+// Xs / Hs.  Rows of the tile are handled as 8 x 16-byte pieces: thread t takes piece cp = t % 8 of rows
+// t / 8 + 32 n (row = 16 k + j), so every global access is a full 16-byte vector.
 template <int NR>
-__device__ __forceinline__ void species_stream_full(const Geom& g, const TileCoord& tc, const PencilGeom& pg,
+__device__ __forceinline__ void species_stream_full(const Geom& g, const TileCoord& tc,
                                                     const double* __restrict__ Ub, const double* __restrict__ rinv_b,
                                                     double* __restrict__ Xs, const double* __restrict__ Ps,
                                                     double* __restrict__ Hs, double* __restrict__ A,
                                                     const UpdArgs& up, const int c_out, const int c_in)
 {
     const int ng = CST_NG;
-    const int tid = threadIdx.x, ti = tid & (TILE - 1), tr = tid >> 4;
-    // ghosted index of the tile zone (i = ti, j = tr, k = 0); row n of this thread is k = n
-    const long long zt = ((long long)(tc.k0 + ng) * g.ey + (tc.j0 + tr + ng)) * g.ex + (tc.i0 + ti + ng);
+    const int tid = threadIdx.x, cp = tid & 7, r0 = tid >> 3;
+    const unsigned long long keep = l2_policy_keep(), strm = l2_policy_stream();
+    // ghosted index (within a component) of tile zone (0, 0, 0)
+    const long long zt = ((long long)(tc.k0 + ng) * g.ey + (tc.j0 + ng)) * g.ex + (tc.i0 + ng);
     if (c_in >= 0) {
         const double* __restrict__ Us = Ub + (long long)c_in * g.comp_g;
+        // core
 #pragma unroll
-        for (int k = 0; k < TILE; ++k) {
-            const long long z = zt + k * g.plane_g;
-            Xs[(k * TILE + tr) * SP_PITCH + ti] = Us[z] * rinv_b[z];
+        for (int n = 0; n < 8; ++n) {
+            const int row = r0 + 32 * n, k = row >> 4, j = row & 15;
+            const long long z = zt + k * g.plane_g + (long long)j * g.ex + 2 * cp;
+            const double2 u = ldg2(Us + z), ri = ldg2_hint(rinv_b + z, keep);
+            double* x = Xs + row * SP_PITCH + 2 * cp;
+            x[0] = u.x * ri.x; x[1] = u.y * ri.y;
         }
+        // y halos (consumer thread = 16 k + i) and z halos (consumer thread = 16 j + i): 768 pieces each
 #pragma unroll
-        for (int d = 0; d < 3; ++d)
-#pragma unroll
-            for (int n = 0; n < 6; ++n) {
-                const long long z = pg.z0[d] + (long long)(n < 3 ? n - 3 : TILE - 3 + n) * pg.stride[d];
-                Hs[(d * 6 + n) * NTHR + tid] = Us[z] * rinv_b[z];
-            }
+        for (int m = 0; m < 3; ++m) {
+            const int idx = tid + NTHR * m, hp = idx & 7, q = (idx >> 3) & 15, n = idx >> 7;
+            const int off = n < 3 ? n - 3 : TILE - 3 + n;
+            const long long zy = zt + q * g.plane_g + (long long)off * g.ex + 2 * hp;
+            const long long zz = zt + off * g.plane_g + (long long)q * g.ex + 2 * hp;
+            const double2 uy = ldg2(Us + zy), ry = ldg2_hint(rinv_b + zy, keep);
+            const double2 uz = ldg2(Us + zz), rz = ldg2_hint(rinv_b + zz, keep);
+            *reinterpret_cast<double2*>(Hs + (6 + n) * NTHR + q * TILE + 2 * hp) = make_double2(uy.x * ry.x, uy.y * ry.y);
+            *reinterpret_cast<double2*>(Hs + (12 + n) * NTHR + q * TILE + 2 * hp) = make_double2(uz.x * rz.x, uz.y * rz.y);
+        }
+        // x halos of this thread's own x pencil (j = tid % 16, k = tid / 16): positions -3 | -2 -1 and 16 17 | 18
+        {
+            const long long zx = zt + (tid >> 4) * g.plane_g + (long long)(tid & 15) * g.ex;
+            const double ul = Us[zx - 3], rl = ldg_hint(rinv_b + zx - 3, keep);
+            const double2 ul2 = ldg2(Us + zx - 2), rl2 = ldg2_hint(rinv_b + zx - 2, keep);
+            const double2 uh2 = ldg2(Us + zx + TILE), rh2 = ldg2_hint(rinv_b + zx + TILE, keep);
+            const double uh = Us[zx + TILE + 2], rh = ldg_hint(rinv_b + zx + TILE + 2, keep);
+            Hs[0 * NTHR + tid] = ul * rl; Hs[1 * NTHR + tid] = ul2.x * rl2.x; Hs[2 * NTHR + tid] = ul2.y * rl2.y;
+            Hs[3 * NTHR + tid] = uh2.x * rh2.x; Hs[4 * NTHR + tid] = uh2.y * rh2.y; Hs[5 * NTHR + tid] = uh * rh;
+        }
     }
     if (c_out >= 0) {
-        const long long plane_a = (long long)g.ny * g.nx;
         const long long ia0 = (long long)tc.b * g.box_a + (long long)c_out * g.comp_a +
-            ((long long)tc.k0 * g.ny + (tc.j0 + tr)) * g.nx + (tc.i0 + ti);
-        const long long iu0 = (long long)tc.b * g.box_g + (long long)c_out * g.comp_g + zt;
-        // batches of four zones: every load of a batch is issued before its first store (the
+            ((long long)tc.k0 * g.ny + tc.j0) * g.nx + tc.i0 + 2 * cp;
+        const long long iu0 = (long long)tc.b * g.box_g + (long long)c_out * g.comp_g + zt + 2 * cp;
+        // batches of four rows: every load of a batch is issued before its first store (the
         // compiler may not move loads over stores that could alias them)
 #pragma unroll
-        for (int k0 = 0; k0 < TILE; k0 += 4) {
-            double av[4], um[4], pv[4][UPD_MAX_EXT];
+        for (int n0 = 0; n0 < 8; n0 += 4) {
+            double2 av[4], um[4], pv[4][UPD_MAX_EXT];
+            long long ia[4], iu[4];
 #pragma unroll
             for (int e = 0; e < 4; ++e) {
-                const int k = k0 + e;
-                av[e] = Ps[(k * TILE + tr) * SP_PITCH + ti];
+                const int row = r0 + 32 * (n0 + e), k = row >> 4, j = row & 15;
+                ia[e] = ia0 + ((long long)k * g.ny + j) * g.nx;
+                iu[e] = iu0 + k * g.plane_g + (long long)j * g.ex;
+                const double* x = Ps + row * SP_PITCH + 2 * cp;
+                av[e] = make_double2(x[0], x[1]);
                 if (NR >= 0) {
-                    um[e] = up.U_m[iu0 + k * g.plane_g];
+                    um[e] = ldg2(up.U_m + iu[e]);
 #pragma unroll
-                    for (int r = 0; r < NR; ++r) pv[e][r] = up.P[r][ia0 + k * plane_a];
+                    for (int r = 0; r < NR; ++r) pv[e][r] = ldg2_hint(up.P[r] + ia[e], strm);
                 }
             }
 #pragma unroll
             for (int e = 0; e < 4; ++e) {
-                const int k = k0 + e;
                 if (NR >= 0) {
-                    double acc = fma(up.ca, av[e], um[e]);
+                    double2 acc = make_double2(fma(up.ca, av[e].x, um[e].x), fma(up.ca, av[e].y, um[e].y));
 #pragma unroll
-                    for (int r = 0; r < NR; ++r) acc = fma(up.c[r], pv[e][r], acc);
-                    up.U_next[iu0 + k * g.plane_g] = acc;
+                    for (int r = 0; r < NR; ++r) {
+                        acc.x = fma(up.c[r], pv[e][r].x, acc.x); acc.y = fma(up.c[r], pv[e][r].y, acc.y);
+                    }
+                    stg2_hint(up.U_next + iu[e], acc, strm);
                 }
-                A[ia0 + k * plane_a] = av[e];
+                stg2_hint(A + ia[e], av[e], strm);
             }
         }
     }
@@ -148,19 +203,11 @@ __device__ __forceinline__ void species_tile_full(const Geom& g, const TileCoord
     double* Xs = sm;
     double* Ps = sm + SP_TILE;
     double* Hs = sm + 2 * SP_TILE;
-    const int ng = CST_NG;
-    const int tid = threadIdx.x, a = tid & (TILE - 1), b = tid >> 4;
-    PencilGeom pg;
-    pg.z0[0] = ((long long)(tc.k0 + b + ng) * g.ey + (tc.j0 + a + ng)) * g.ex + (tc.i0 + ng);
-    pg.z0[1] = ((long long)(tc.k0 + b + ng) * g.ey + (tc.j0 + ng)) * g.ex + (tc.i0 + a + ng);
-    pg.z0[2] = ((long long)(tc.k0 + ng) * g.ey + (tc.j0 + b + ng)) * g.ex + (tc.i0 + a + ng);
-    pg.stride[0] = 1; pg.stride[1] = g.ex; pg.stride[2] = g.plane_g;
-
     double fmc[TILE + 1], fmn[TILE + 1];
     load_fm(fm_tile, 0, fmc);
     for (int s = 0; s <= g.nspec; ++s) {
         __syncthreads();                                // z sweep of species s-1 done; Xs, Hs free
-        species_stream_full<NR>(g, tc, pg, Ub, rinv_b, Xs, Ps, Hs, A, up,
+        species_stream_full<NR>(g, tc, Ub, rinv_b, Xs, Ps, Hs, A, up,
                                 s > 0 ? 5 + s - 1 : -1, s < g.nspec ? 5 + s : -1);
         if (s == g.nspec) break;
         __syncthreads();
