@@ -53,7 +53,9 @@ def alg_bytes(cfg):
     fill = 2.0 * (G - 1.0) * N * 8.0                 # read source + write ghost, full shell
     adv = (G3 + 4.0) * N * 8.0                       # U (+3-deep face ghosts), A_old^m, A_old^other, A_new, U_next
     cfl = 5.0 * 8.0                                  # hydro components of the interior
-    return dict(fill=fill, advance=adv, cfl=cfl, step=fill + adv + cfl, G=G, G3=G3)
+    # the advance runs as two kernels: the 5 hydro components and the nspec species components
+    return dict(fill=fill, advance=adv, cfl=cfl, step=fill + adv + cfl, G=G, G3=G3,
+                advance_hydro=(G3 + 4.0) * 5 * 8.0, advance_species=(G3 + 4.0) * (N - 5) * 8.0)
 
 
 def measured_peaks():
@@ -182,6 +184,25 @@ def run_reference(args, cfg, rank):
     print(json.dumps(line), flush=True)
 
 
+# ------------------------------------------------------------------------------- multi-rank ----
+def allreduce_scalar(x, op, device, world):
+    """MIN / MAX of a host scalar over the ranks (dt: MIN, device time: MAX).  The path shards as
+    independent replicas of the box lattice: these two scalars are the only
+    things that cross ranks.  Works with any torch.distributed backend (nccl on GPUs, gloo in tests)."""
+    if world <= 1:
+        return float(x)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([float(x)], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MIN if op == "min" else dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def aggregate_value(zones_per_rank, world, ms_step_max):
+    """whole-job zone-updates/s: every rank advances its own zones_per_rank zones in ms_step_max."""
+    return zones_per_rank * world / (ms_step_max * 1e-3)
+
+
 # -------------------------------------------------------------------------------------- main ----
 def main():
     args = parse()
@@ -228,17 +249,15 @@ def main():
     dt_dev = torch.zeros(1, dtype=torch.float64, device=dev)
     ctx.fill_ghosts(U)
     dt = ctx.cfl_dt(U, 0.5)
-    if world > 1:
-        t = torch.tensor([dt], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MIN)
-        dt = float(t.item())
+    dt = allreduce_scalar(dt, "min", dev, world)
     # A_old buffers hold plausible values: A of the initial state and a perturbation of it
     ctx.advance_A(U, A_old0)
     A_old1.copy_(A_old0).mul_(0.9)
     w = [0.5 * dt, 0.5 * dt]
 
     ev = lambda: torch.cuda.Event(enable_timing=True)
-    k_ev = []
+    k_ev, k_ms2 = [], []
+    ctx.set_timing(True)      # CUDA events around the two kernels of the advance, on this stream (cst.h)
 
     def step(timed):
         ctx.fill_ghosts(U)
@@ -268,31 +287,38 @@ def main():
         step(True)
     s1.record()
     sync_all()
+    k_ms2.append(ctx.last_advance_ms())      # (hydro, species) of the last timed step
     t_wall1 = time.time()
     launches = ctx.launch_count() - l0
     ms = s0.elapsed_time(s1)
-    if world > 1:
-        t = torch.tensor([ms], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
+    ms = allreduce_scalar(ms, "max", dev, world)
     clocks = sampler.stop(t_wall0, t_wall1) if sampler else None
     ms_step = ms / args.steps
-    value = zones * world / (ms_step * 1e-3)
+    value = aggregate_value(zones, world, ms_step)
     k_ms = float(np.mean([a.elapsed_time(b) for a, b in k_ev]))
 
-    # ---- roofline of the dominant kernel (the fused advance+update kernel) ------------------
+    # ---- roofline of the dominant kernel: k_advect_species (the species components of the fused
+    #      A + node update); k_advect_hydro and the whole advance call are reported beside it
     ab = alg_bytes(cfg)
     peak, peak_src = measured_peaks()
-    achieved = ab["advance"] * zones / (k_ms * 1e-3) / 1e9
+    ms_hydro, ms_species = k_ms2[-1]
     traffic = None
     try:
         tj = json.load(open(os.path.join(ROOT, "profiles", "traffic.json")))
-        traffic = tj.get(f"configs[{cfg['index']}]", {}).get("advance_dram_bytes_per_launch")
+        traffic = tj.get(f"configs[{cfg['index']}]", {}).get("k_advect_species_dram_bytes_per_launch")
     except Exception:
         pass
-    roofline = {"bound": "hbm", "kernel": "advance_A_update (S1-S5)", "achieved": achieved, "peak": peak,
+    if N > 5:
+        dom, dom_ms, dom_bytes = "k_advect_species<2> (S1-S5, species components)", ms_species, ab["advance_species"]
+    else:
+        dom, dom_ms, dom_bytes = "k_advect_hydro<2> (S1-S5, hydro components)", ms_hydro, ab["advance_hydro"]
+    achieved = dom_bytes * zones / (dom_ms * 1e-3) / 1e9
+    roofline = {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak,
                 "unit": "GB/s", "frac": achieved / peak, "traffic": traffic, "peak_source": peak_src,
-                "alg_bytes_per_zone": ab["advance"], "kernel_ms": k_ms,
+                "alg_bytes_per_zone": dom_bytes, "kernel_ms": dom_ms,
+                "other_kernels": {"k_advect_hydro_ms": ms_hydro, "k_advect_species_ms": ms_species,
+                                  "advance_call_ms": k_ms,
+                                  "advance_call_frac": ab["advance"] * zones / (k_ms * 1e-3) / 1e9 / peak},
                 "whole_step_frac": ab["step"] * zones / (ms_step * 1e-3) / 1e9 / peak}
 
     # ---- end to end through the C ABI with HOST buffers (H2D + D2H inside the timed region) --
@@ -317,10 +343,7 @@ def main():
             ctx.step_host(U_host, A_host, Un_host, U, U_next, A_new, dt)
         sync_all()
         sec = (time.perf_counter() - t0) / n_e2e
-        if world > 1:
-            t = torch.tensor([sec], dtype=torch.float64, device=dev)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            sec = float(t.item())
+        sec = allreduce_scalar(sec, "max", dev, world)
         e2e = {"value": zones * world / sec, "unit": UNIT, "h2d_bytes_per_step": ubytes,
                "d2h_bytes_per_step": abytes + ubytes, "steps": n_e2e, "host_memory": "pinned" if pinned else "pageable",
                "call": "cst_step_host (H2D U, fill_ghosts, advance_A_update, D2H A and U_next)"}

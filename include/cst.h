@@ -109,6 +109,13 @@ int cst_step_host(cst_ctx* ctx, const double* U_host, double* A_host, double* U_
                   double* U_dev, double* U_next_dev, double* A_dev,
                   double dt_m, void* stream);   /* needs the workspace, see cst_set_workspace */
 
+/* Measurement aid (bench.py roofline): with timing on, cst_advance_A / cst_advance_A_update record CUDA
+ * events on the caller's stream around their two kernels (hydro components, species components);
+ * cst_last_advance_ms waits for the last recorded call and returns the two durations in
+ * milliseconds (CST_EINVAL if timing was never switched on).  Off by default. */
+int cst_set_timing(cst_ctx* ctx, int on);
+int cst_last_advance_ms(cst_ctx* ctx, double* ms_hydro, double* ms_species);
+
 /* Number of kernel launches issued through this context since creation (for bench accounting). */
 long long cst_launch_count(const cst_ctx* ctx);
 

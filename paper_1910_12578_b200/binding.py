@@ -13,7 +13,7 @@ MAX_QUAD = 4
 
 EXPORTS = ["cst_create", "cst_destroy", "cst_workspace_bytes", "cst_set_workspace", "cst_fill_ghosts", "cst_advance_A", "cst_sdc_update",
            "cst_advance_A_update", "cst_cfl_dt_device", "cst_cfl_dt", "cst_step_host",
-           "cst_launch_count", "cst_strerror", "cst_version"]
+           "cst_set_timing", "cst_last_advance_ms", "cst_launch_count", "cst_strerror", "cst_version"]
 
 
 class CstParams(C.Structure):
@@ -57,6 +57,8 @@ def load():
     lib.cst_cfl_dt_device.argtypes = [_vp, _vp, C.c_double, _vp, _vp]
     lib.cst_cfl_dt.argtypes = [_vp, _vp, C.c_double, _dp, _vp]
     lib.cst_step_host.argtypes = [_vp, _vp, _vp, _vp, _vp, _vp, _vp, C.c_double, _vp]
+    lib.cst_set_timing.argtypes = [_vp, C.c_int]
+    lib.cst_last_advance_ms.argtypes = [_vp, _dp, _dp]
     lib.cst_launch_count.argtypes = [_vp]
     lib.cst_launch_count.restype = C.c_longlong
     lib.cst_strerror.argtypes = [C.c_int]
@@ -176,6 +178,14 @@ class Context:
         self._check(self.lib.cst_step_host(self._h, _ptr(U_host), _ptr(A_host), _ptr(U_next_host), _ptr(U_dev),
                                            _ptr(U_next_dev), _ptr(A_dev), float(dt_m), _stream(stream)),
                     "cst_step_host")
+
+    def set_timing(self, on):
+        self._check(self.lib.cst_set_timing(self._h, int(bool(on))), "cst_set_timing")
+
+    def last_advance_ms(self):
+        a, b = C.c_double(0.0), C.c_double(0.0)
+        self._check(self.lib.cst_last_advance_ms(self._h, C.byref(a), C.byref(b)), "cst_last_advance_ms")
+        return a.value, b.value
 
     def launch_count(self):
         return int(self.lib.cst_launch_count(self._h))

@@ -38,9 +38,12 @@ int launch_advance_A(cst_ctx* ctx, const double* U, double* A, double* U_next, d
     up.nr = -1; up.U_m = U; up.A_base = A;
     bool split = false;
     if (fused && !make_upd(up, U, A, U_next, dt_m, A_old_m, q)) { up.nr = -1; split = true; }
+    if (ctx->timing) cudaEventRecord(ctx->ev[0], st);
     int rc = launch_advect_hydro(ctx, U, A, up, st);
     if (rc) return rc;
+    if (ctx->timing) cudaEventRecord(ctx->ev[1], st);
     rc = launch_advect_species(ctx, U, A, up, st);
+    if (ctx->timing) cudaEventRecord(ctx->ev[2], st);
     if (rc || !split) return rc;
     // too many distinct arrays for the fused epilogue: A first, then the plain update kernel
     return launch_sdc_update(ctx, U_next, U, dt_m, A, A_old_m, q, st);

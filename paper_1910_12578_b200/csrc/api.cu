@@ -61,6 +61,8 @@ extern "C" int cst_create(const cst_params* p, cst_ctx** out)
     g.box_a = g.comp_a * g.nvar;
     c->launches = 0;
     c->ws = nullptr; c->ws_bytes = 0;
+    c->timing = 0;
+    for (int n = 0; n < 3; ++n) c->ev[n] = nullptr;
     int dev = 0;
     cudaError_t e = cudaGetDevice(&dev);
     if (e == cudaSuccess) e = cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, dev);
@@ -74,6 +76,7 @@ extern "C" int cst_destroy(cst_ctx* c)
 {
     if (!c) return CST_EINVAL;
     cudaFree(c->d_scratch);
+    for (int n = 0; n < 3; ++n) if (c->ev[n]) cudaEventDestroy(c->ev[n]);
     delete c;
     return CST_OK;
 }
@@ -179,6 +182,28 @@ extern "C" int cst_step_host(cst_ctx* c, const double* U_host, double* A_host, d
     if (e == cudaSuccess) e = cudaMemcpyAsync(U_next_host, U_next_dev, ub, cudaMemcpyDeviceToHost, st);
     if (e == cudaSuccess) e = cudaStreamSynchronize(st);
     return e == cudaSuccess ? CST_OK : cuda_fail(e);
+}
+
+extern "C" int cst_set_timing(cst_ctx* c, int on)
+{
+    if (!c) return CST_EINVAL;
+    if (on && !c->ev[0])
+        for (int n = 0; n < 3; ++n)
+            if (cudaEventCreate(&c->ev[n]) != cudaSuccess) return cuda_fail(cudaGetLastError());
+    c->timing = on ? 1 : 0;
+    return CST_OK;
+}
+
+extern "C" int cst_last_advance_ms(cst_ctx* c, double* ms_hydro, double* ms_species)
+{
+    if (!c || !ms_hydro || !ms_species || !c->ev[0]) return CST_EINVAL;
+    cudaError_t e = cudaEventSynchronize(c->ev[2]);
+    float a = 0.f, b = 0.f;
+    if (e == cudaSuccess) e = cudaEventElapsedTime(&a, c->ev[0], c->ev[1]);
+    if (e == cudaSuccess) e = cudaEventElapsedTime(&b, c->ev[1], c->ev[2]);
+    if (e != cudaSuccess) return cuda_fail(e);
+    *ms_hydro = a; *ms_species = b;
+    return CST_OK;
 }
 
 extern "C" long long cst_launch_count(const cst_ctx* c) { return c ? c->launches : -1; }

@@ -33,6 +33,8 @@ struct cst_ctx {
     long long ws_bytes;
     long long launches;
     int sm_count;
+    int timing;              // cst_set_timing: record events around the kernels of the advance calls
+    cudaEvent_t ev[3];       // before hydro, between hydro and species, after species
 };
 
 struct UpdArgs;
