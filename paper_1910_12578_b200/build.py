@@ -35,7 +35,8 @@ def build(force=False, verbose=False):
     from concurrent.futures import ThreadPoolExecutor
     objdir = os.path.join(HERE, "build")
     os.makedirs(objdir, exist_ok=True)
-    cflags = [f for f in FLAGS if f != "--shared"] + (["-Xptxas", "-v"] if verbose else [])
+    cflags = [f for f in FLAGS if f != "--shared"] + (["-Xptxas", "-v"] if verbose else []) + \
+        os.environ.get("CST_NVCC_EXTRA", "").split()
 
     def compile_one(src):
         obj = os.path.join(objdir, os.path.basename(src)[:-3] + ".o")

@@ -17,6 +17,18 @@
 // Shared memory: 2 x 16*16*17 + 18*256 doubles = 106.5 KB per CTA, so two CTAs (16 warps) share an SM.
 #include "sweep.cuh"
 #include "tile.cuh"
+#include "species_group.cuh"
+
+#ifndef SPG_G
+#define SPG_G 1        // species per pass of the full-tile fast path
+#endif
+#ifndef SPG_PP
+#define SPG_PP 1       // pencils per thread of the full-tile fast path (CTA = 256 / SPG_PP threads)
+#endif
+#define SPG_NT (NTHR / SPG_PP)
+#ifndef SPG_CTAS
+#define SPG_CTAS 2     // resident CTAs per SM the fast path is sized for (128 registers per thread)
+#endif
 
 #define SP_PITCH 17
 #define SP_TILE (TILE * TILE * SP_PITCH)
@@ -336,21 +348,42 @@ k_advect_species(Geom g, TileGeom tg, const double* __restrict__ U, double* __re
     }
 }
 
+// every tile of every box is a full 16^3: CTAs of SPG_NT threads, SPG_PP pencils per thread (species_group.cuh)
+template <int NR>
+__global__ void __launch_bounds__(SPG_NT, SPG_CTAS)
+k_advect_species_full(Geom g, TileGeom tg, const double* __restrict__ U, double* __restrict__ A,
+                      const double* __restrict__ rinv, const double* __restrict__ Fm, UpdArgs up)
+{
+    extern __shared__ double sm[];
+    const TileCoord tc = tile_coord(g, tg, blockIdx.x);
+    spg_tile<SPG_G, SPG_PP, NR>(g, tc, U + (long long)tc.b * g.box_g, rinv + (long long)tc.b * g.comp_g,
+                                Fm + tc.tile * 3LL * (TILE + 1) * NTHR, A, up, sm);
+}
+
 template <int NR>
 static int launch_species_nr(cst_ctx* ctx, const double* U, double* A, const UpdArgs& up, cudaStream_t st)
 {
     const Geom& g = ctx->g;
     const TileGeom tg = make_tile_geom(g);
-    const size_t smem = (2ull * SP_TILE + SP_HALO) * sizeof(double);
+    const double* rinv = ctx->ws;
+    const double* Fm = ctx->ws + ws_rinv_doubles(g);
     static bool attr_set = false;
+    const size_t smem_full = 2ull * SPG_G * SPG_TILE * sizeof(double);
+    const size_t smem = (2ull * SP_TILE + SP_HALO) * sizeof(double);
     if (!attr_set) {
-        if (cudaFuncSetAttribute(k_advect_species<NR>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
+        if (cudaFuncSetAttribute(k_advect_species<NR>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess ||
+            cudaFuncSetAttribute(k_advect_species_full<NR>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_full) != cudaSuccess)
             return CST_ECUDA;
         attr_set = true;
     }
-    const double* rinv = ctx->ws;
-    const double* Fm = ctx->ws + ws_rinv_doubles(g);
-    k_advect_species<NR><<<(unsigned)tg.ntiles, NTHR, smem, st>>>(g, tg, U, A, rinv, Fm, up);
+    // 16-byte vector accesses of the fast path need even row lengths (true for multiples of 16) and aligned bases
+    const bool all_full = (g.nx % TILE == 0) && (g.ny % TILE == 0) && (g.nz % TILE == 0) &&
+                          ((((uintptr_t)U | (uintptr_t)A | (uintptr_t)up.U_next | (uintptr_t)up.P[0] |
+                             (uintptr_t)up.P[1] | (uintptr_t)up.P[2]) & 15) == 0);
+    if (all_full)
+        k_advect_species_full<NR><<<(unsigned)tg.ntiles, SPG_NT, smem_full, st>>>(g, tg, U, A, rinv, Fm, up);
+    else
+        k_advect_species<NR><<<(unsigned)tg.ntiles, NTHR, smem, st>>>(g, tg, U, A, rinv, Fm, up);
     ctx->launches++;
     return cudaGetLastError() == cudaSuccess ? CST_OK : CST_ECUDA;
 }

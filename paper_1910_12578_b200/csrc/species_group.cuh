@@ -1,0 +1,316 @@
+// species_group.cuh -- fast path of k_advect_species for full 16^3 tiles: G species per pass.
+//
+// A CTA of 256 / PP threads owns one tile; every thread marches PP pencils of G species AT ONCE:
+// G x PP independent PPM windows in registers give each warp the instruction-level parallelism that
+// the FP64 pipe latency needs, the face mass fluxes Fm and 1/rho are fetched once per G species, and
+// 2 G x 16*16*17 doubles of shared memory per CTA leave room for several CTAs per SM, whose
+// streaming phases (stage the next group / write out the previous one) overlap the sweeps of the others.
+// The sweep is ONE body of code with the direction as a run-time argument (strides, bases), executed
+// three times, and its march is a loop over groups of four zones: the kernel stays in the
+// instruction cache.
+// Same arithmetic, zone for zone, as species_sweep (advect_species.cu) and as the oracle's S1-S5.
+#pragma once
+#include "sweep.cuh"
+#include "tile.cuh"
+
+#define SPG_PITCH 17
+#define SPG_TILE (TILE * TILE * SPG_PITCH)
+
+__device__ __forceinline__ unsigned long long spg_policy_keep()
+{
+    unsigned long long p;
+    asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(p));
+    return p;
+}
+__device__ __forceinline__ unsigned long long spg_policy_stream()
+{
+    unsigned long long p;
+    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
+    return p;
+}
+__device__ __forceinline__ double spg_ldg(const double* a, unsigned long long pol)
+{
+    double v;
+    asm volatile("ld.global.nc.L2::cache_hint.f64 %0, [%1], %2;" : "=d"(v) : "l"(a), "l"(pol));
+    return v;
+}
+__device__ __forceinline__ double2 spg_ldg2(const double* a, unsigned long long pol)
+{
+    double2 v;
+    asm volatile("ld.global.nc.L2::cache_hint.v2.f64 {%0,%1}, [%2], %3;" : "=d"(v.x), "=d"(v.y) : "l"(a), "l"(pol));
+    return v;
+}
+__device__ __forceinline__ double2 spg_ldg2(const double* a)
+{
+    double2 v;
+    asm volatile("ld.global.nc.v2.f64 {%0,%1}, [%2];" : "=d"(v.x), "=d"(v.y) : "l"(a));
+    return v;
+}
+__device__ __forceinline__ void spg_stg2(double* a, double2 v, unsigned long long pol)
+{
+    asm volatile("st.global.L2::cache_hint.v2.f64 [%0], {%1,%2}, %3;" :: "l"(a), "d"(v.x), "d"(v.y), "l"(pol) : "memory");
+}
+
+// geometry of pencil number q of this thread (pencil id = threadIdx.x + q * blockDim.x) in direction d
+// (run-time d, uniform over the CTA)
+struct SpgPencil {
+    long long z0;      // ghosted index (within a component of the box) of pencil position 0
+    long long stride;  // ghosted stride along the pencil
+    int s0, sst;       // shared-memory index of position 0 and stride along the pencil
+    double nrd;        // -1/delta_d
+};
+
+__device__ __forceinline__ SpgPencil spg_pencil(const Geom& g, const TileCoord& tc, const int d, const int pid)
+{
+    const int ng = CST_NG;
+    const int a = pid & (TILE - 1), b = pid >> 4;
+    SpgPencil pc;
+    const long long zt = ((long long)(tc.k0 + ng) * g.ey + (tc.j0 + ng)) * g.ex + (tc.i0 + ng);
+    if (d == 0) {           // (a, b) = (j, k)
+        pc.z0 = zt + b * g.plane_g + (long long)a * g.ex; pc.stride = 1;
+        pc.s0 = (b * TILE + a) * SPG_PITCH; pc.sst = 1; pc.nrd = -g.rdx;
+    } else if (d == 1) {    // (a, b) = (i, k)
+        pc.z0 = zt + b * g.plane_g + a; pc.stride = g.ex;
+        pc.s0 = (b * TILE) * SPG_PITCH + a; pc.sst = SPG_PITCH; pc.nrd = -g.rdy;
+    } else {                // (a, b) = (i, j)
+        pc.z0 = zt + (long long)b * g.ex + a; pc.stride = g.plane_g;
+        pc.s0 = b * SPG_PITCH + a; pc.sst = TILE * SPG_PITCH; pc.nrd = -g.rdz;
+    }
+    return pc;
+}
+
+// raw halo operands of the PP pencils: positions -3..-1 (n = 0..2) and 16..18 (n = 3..5)
+template <int G, int PP>
+struct SpgHaloRaw {
+    double u[G][PP][6];
+    double r[PP][6];
+};
+
+template <int G, int PP>
+__device__ __forceinline__ void spg_halo_load(const Geom& g, const double* __restrict__ Ub,
+                                              const double* __restrict__ rinv_b, const SpgPencil (&pc)[PP],
+                                              const int c0, const int ng_, SpgHaloRaw<G, PP>& h)
+{
+    const unsigned long long keep = spg_policy_keep();
+#pragma unroll
+    for (int q = 0; q < PP; ++q)
+#pragma unroll
+        for (int n = 0; n < 6; ++n) {
+            const long long z = pc[q].z0 + (long long)(n < 3 ? n - 3 : TILE - 3 + n) * pc[q].stride;
+            h.r[q][n] = spg_ldg(rinv_b + z, keep);
+#pragma unroll
+            for (int s = 0; s < G; ++s)
+                h.u[s][q][n] = (s < ng_) ? Ub[(long long)(c0 + s) * g.comp_g + z] : 0.0;
+        }
+}
+
+// One sweep of G species x PP pencils along direction d (run-time): S2 window march, F = Fm * X(upwind),
+// flux difference into the partial-sum arrays.  first = true for the x sweep (the partial sum starts).
+// hx[s][q][n]: halo X values (n = 0..2: positions -3..-1, n = 3..5: positions 16..18).
+template <int G, int PP>
+__device__ __forceinline__ void spg_sweep(const SpgPencil (&pc)[PP], const bool first, const double* __restrict__ Xs,
+                                          double* __restrict__ Ps, const double* __restrict__ fm_d,
+                                          const double (&hx)[G][PP][6])
+{
+    const int sst = pc[0].sst;
+    const double nrd = pc[0].nrd;
+    const int nthr = NTHR / PP;
+    const unsigned long long keep = spg_policy_keep();
+    PpmWindow w[G][PP];
+    double Fprev[G][PP];
+    const double* __restrict__ fm = fm_d + threadIdx.x;          // pencil q: + q * nthr
+
+    auto face = [&](const int s, const int q, const double fmc) -> double {
+        return fmc * (sign_bit(fmc) ? w[s][q].qm : w[s][q].qpL);
+    };
+    auto zone = [&](const int s, const int q, const int qoff, const double dF) {
+        double* p = Ps + s * SPG_TILE + pc[q].s0 + qoff;
+        const double old = first ? 0.0 : *p;
+        *p = fma(dF, nrd, old);
+    };
+    auto xval = [&](const int s, const int q, const int off) -> double { return Xs[s * SPG_TILE + pc[q].s0 + off]; };
+
+    // ---- prologue: pencil positions -3 .. 3 (faces 0, 1; zone 0)
+    double f0[PP], f1[PP], fn[PP][4];
+#pragma unroll
+    for (int q = 0; q < PP; ++q) {
+        f0[q] = spg_ldg(fm + q * nthr, keep); f1[q] = spg_ldg(fm + q * nthr + NTHR, keep);
+#pragma unroll
+        for (int e = 0; e < 4; ++e) fn[q][e] = spg_ldg(fm + q * nthr + (2 + e) * NTHR, keep);
+    }
+#pragma unroll
+    for (int s = 0; s < G; ++s)
+#pragma unroll
+        for (int q = 0; q < PP; ++q) {
+            PpmWindow& ww = w[s][q];
+            ww.start(hx[s][q][0]); ww.warm1(hx[s][q][1]); ww.warm2(hx[s][q][2]);
+            ww.warm3(xval(s, q, 0));
+            ww.push(xval(s, q, sst));
+            ww.push(xval(s, q, 2 * sst));
+            const double F0 = face(s, q, f0[q]);
+            ww.push(xval(s, q, 3 * sst));
+            const double F1 = face(s, q, f1[q]);
+            zone(s, q, 0, F1 - F0);
+            Fprev[s][q] = F1;
+        }
+    // ---- positions 4 .. 15: three groups of four (faces p-2, zones p-3)
+#pragma unroll 1
+    for (int it = 1; it <= 3; ++it) {
+        double fc[PP][4];
+#pragma unroll
+        for (int q = 0; q < PP; ++q)
+#pragma unroll
+            for (int e = 0; e < 4; ++e) {
+                fc[q][e] = fn[q][e];
+                if (it < 3 || e < 3) fn[q][e] = spg_ldg(fm + q * nthr + (4 * it + 2 + e) * NTHR, keep);
+            }
+        const int p0 = 4 * it * sst;
+#pragma unroll
+        for (int e = 0; e < 4; ++e)
+#pragma unroll
+            for (int s = 0; s < G; ++s)
+#pragma unroll
+                for (int q = 0; q < PP; ++q) {
+                    w[s][q].push(xval(s, q, p0 + e * sst));
+                    const double F = face(s, q, fc[q][e]);
+                    zone(s, q, p0 + (e - 3) * sst, F - Fprev[s][q]);
+                    Fprev[s][q] = F;
+                }
+    }
+    // ---- epilogue: positions 16 .. 18 (faces 14..16, zones 13..15)
+#pragma unroll
+    for (int e = 0; e < 3; ++e)
+#pragma unroll
+        for (int s = 0; s < G; ++s)
+#pragma unroll
+            for (int q = 0; q < PP; ++q) {
+                w[s][q].push(hx[s][q][3 + e]);
+                const double F = face(s, q, fn[q][e]);
+                zone(s, q, (13 + e) * sst, F - Fprev[s][q]);
+                Fprev[s][q] = F;
+            }
+}
+
+// streaming phase: write out the n_out species from c_out0 (A and, fused, U_next) out of Ps, stage the
+// n_in species from c_in0 into Xs.  Rows of the tile are handled as 8 x 16-byte pieces: thread t takes
+// piece cp = t % 8 of rows t / 8 + (32 / PP) n (row = 16 k + j): every global access is a 16-byte vector.
+template <int G, int PP, int NR>
+__device__ __forceinline__ void spg_stream(const Geom& g, const TileCoord& tc, const double* __restrict__ Ub,
+                                           const double* __restrict__ rinv_b, double* __restrict__ Xs,
+                                           const double* __restrict__ Ps, double* __restrict__ A, const UpdArgs& up,
+                                           const int c_out0, const int n_out, const int c_in0, const int n_in)
+{
+    const int ng = CST_NG;
+    const int tid = threadIdx.x, cp = tid & 7, r0 = tid >> 3;
+    constexpr int RS = 32 / PP, NROW = 8 * PP;          // row stride and rows per thread
+    const unsigned long long keep = spg_policy_keep(), strm = spg_policy_stream();
+    const long long zt = ((long long)(tc.k0 + ng) * g.ey + (tc.j0 + ng)) * g.ex + (tc.i0 + ng) + 2 * cp;
+    if (n_in > 0) {
+        // one batch: 1/rho and the G species of all eight rows
+        double2 ri[NROW], u[G][NROW];
+#pragma unroll
+        for (int n = 0; n < NROW; ++n) {
+            const int row = r0 + RS * n, k = row >> 4, j = row & 15;
+            const long long z = zt + k * g.plane_g + (long long)j * g.ex;
+            ri[n] = spg_ldg2(rinv_b + z, keep);
+#pragma unroll
+            for (int s = 0; s < G; ++s)
+                if (s < n_in) u[s][n] = spg_ldg2(Ub + (long long)(c_in0 + s) * g.comp_g + z);
+        }
+#pragma unroll
+        for (int n = 0; n < NROW; ++n) {
+            double* x = Xs + (r0 + RS * n) * SPG_PITCH + 2 * cp;
+#pragma unroll
+            for (int s = 0; s < G; ++s)
+                if (s < n_in) { x[s * SPG_TILE] = u[s][n].x * ri[n].x; x[s * SPG_TILE + 1] = u[s][n].y * ri[n].y; }
+        }
+    }
+    if (n_out > 0) {
+        const long long ia0 = (long long)tc.b * g.box_a + ((long long)tc.k0 * g.ny + tc.j0) * g.nx + tc.i0 + 2 * cp;
+        const long long iu0 = (long long)tc.b * g.box_g + zt;
+#pragma unroll 1
+        for (int s = 0; s < n_out; ++s) {
+            const long long ias = ia0 + (long long)(c_out0 + s) * g.comp_a;
+            const long long ius = iu0 + (long long)(c_out0 + s) * g.comp_g;
+            const double* __restrict__ pss = Ps + s * SPG_TILE;
+            // batches of four rows: every load of a batch is issued before its first store
+#pragma unroll
+            for (int n0 = 0; n0 < NROW; n0 += 4) {
+                double2 um[4], pv[4][UPD_MAX_EXT];
+#pragma unroll
+                for (int e = 0; e < 4; ++e) {
+                    const int row = r0 + RS * (n0 + e), k = row >> 4, j = row & 15;
+                    if (NR >= 0) {
+                        um[e] = spg_ldg2(up.U_m + ius + k * g.plane_g + (long long)j * g.ex);
+#pragma unroll
+                        for (int r = 0; r < NR; ++r)
+                            pv[e][r] = spg_ldg2(up.P[r] + ias + ((long long)k * g.ny + j) * g.nx, strm);
+                    }
+                }
+#pragma unroll
+                for (int e = 0; e < 4; ++e) {
+                    const int row = r0 + RS * (n0 + e), k = row >> 4, j = row & 15;
+                    const double* x = pss + row * SPG_PITCH + 2 * cp;
+                    const double2 av = make_double2(x[0], x[1]);
+                    if (NR >= 0) {
+                        double2 acc = make_double2(fma(up.ca, av.x, um[e].x), fma(up.ca, av.y, um[e].y));
+#pragma unroll
+                        for (int r = 0; r < NR; ++r) {
+                            acc.x = fma(up.c[r], pv[e][r].x, acc.x); acc.y = fma(up.c[r], pv[e][r].y, acc.y);
+                        }
+                        spg_stg2(up.U_next + ius + k * g.plane_g + (long long)j * g.ex, acc, strm);
+                    }
+                    spg_stg2(A + ias + ((long long)k * g.ny + j) * g.nx, av, strm);
+                }
+            }
+        }
+    }
+}
+
+// all species of one full tile, G at a time
+template <int G, int PP, int NR>
+__device__ __forceinline__ void spg_tile(const Geom& g, const TileCoord& tc, const double* __restrict__ Ub,
+                                         const double* __restrict__ rinv_b, const double* __restrict__ fm_tile,
+                                         double* __restrict__ A, const UpdArgs& up, double* __restrict__ sm)
+{
+    double* Xs = sm;                    // [G][SPG_TILE]  X of the tile core
+    double* Ps = sm + G * SPG_TILE;     // [G][SPG_TILE]  A under construction
+    const int tid = threadIdx.x, nthr = NTHR / PP;
+    int c_prev = 0, n_prev = 0;
+#pragma unroll 1
+    for (int s0 = 0; s0 < g.nspec; s0 += G) {
+        const int n_in = min(G, g.nspec - s0), c_in = 5 + s0;
+        __syncthreads();                                // z sweep of the previous group done
+        spg_stream<G, PP, NR>(g, tc, Ub, rinv_b, Xs, Ps, A, up, c_prev, n_prev, c_in, n_in);
+        // halo operands of the x sweep (products formed after the barrier, when the loads have landed)
+        SpgHaloRaw<G, PP> hr;
+        SpgPencil pc[PP];
+#pragma unroll
+        for (int q = 0; q < PP; ++q) pc[q] = spg_pencil(g, tc, 0, tid + q * nthr);
+        spg_halo_load<G, PP>(g, Ub, rinv_b, pc, c_in, n_in, hr);
+        __syncthreads();
+#pragma unroll 1
+        for (int d = 0; d < 3; ++d) {
+            double hx[G][PP][6];
+#pragma unroll
+            for (int s = 0; s < G; ++s)
+#pragma unroll
+                for (int q = 0; q < PP; ++q)
+#pragma unroll
+                    for (int n = 0; n < 6; ++n) hx[s][q][n] = hr.u[s][q][n] * hr.r[q][n];
+            SpgPencil pcd[PP];
+#pragma unroll
+            for (int q = 0; q < PP; ++q) pcd[q] = pc[q];
+            if (d < 2) {                                // operands of the next sweep: in flight during this one
+#pragma unroll
+                for (int q = 0; q < PP; ++q) pc[q] = spg_pencil(g, tc, d + 1, tid + q * nthr);
+                spg_halo_load<G, PP>(g, Ub, rinv_b, pc, c_in, n_in, hr);
+            }
+            spg_sweep<G, PP>(pcd, d == 0, Xs, Ps, fm_tile + (d * (TILE + 1)) * NTHR, hx);
+            if (d < 2) __syncthreads();
+        }
+        c_prev = c_in; n_prev = n_in;
+    }
+    __syncthreads();
+    spg_stream<G, PP, NR>(g, tc, Ub, rinv_b, Xs, Ps, A, up, c_prev, n_prev, 0, 0);
+}

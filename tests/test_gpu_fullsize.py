@@ -16,6 +16,9 @@ TOL = 1e-12
 
 
 def need_gb(gb):
+    import gc
+    gc.collect()
+    torch.cuda.empty_cache()
     free, _ = torch.cuda.mem_get_info()
     if free < gb * 1e9:
         pytest.skip(f"needs {gb} GB of free device memory, has {free / 1e9:.0f}")
@@ -68,12 +71,12 @@ def check_samples(cfg, samples, sub=16):
 def test_configs3_512_sampled():
     need_gb(110)
     cfg = wl.make_config(3)
-    s = [(0, 0, 0, 0), (0, 496, 496, 496), (0, 248, 8, 500), (0, 100, 300, 16), (0, 8, 250, 250), (0, 333, 77, 129)]
+    s = [(0, 0, 0, 0), (0, 496, 496, 496), (0, 248, 8, 496), (0, 100, 300, 16), (0, 8, 250, 250), (0, 333, 77, 129)]
     check_samples(cfg, s)
 
 
 def test_configs4_boxes_sampled():
-    need_gb(130)
+    need_gb(122)
     cfg = wl.make_config(4)
     # boxes at the reflecting z walls, at periodic x/y wraps and in the interior; sub-boxes touching box faces
     s = [(0, 0, 0, 0), (511, 48, 48, 48), (16 * 8 * 3 + 5, 48, 0, 20), (130, 20, 48, 0), (257, 24, 24, 24), (15, 0, 30, 48)]
