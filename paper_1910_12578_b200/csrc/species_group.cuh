@@ -15,6 +15,7 @@
 
 #define SPG_PITCH 17
 #define SPG_TILE (TILE * TILE * SPG_PITCH)
+#define SPG_HALO (3 * 6 * NTHR)         // halo X values of one species: [direction][n][pencil id]
 
 __device__ __forceinline__ unsigned long long spg_policy_keep()
 {
@@ -131,12 +132,15 @@ __device__ __forceinline__ void spg_sweep(const SpgPencil (&pc)[PP], const bool 
     auto xval = [&](const int s, const int q, const int off) -> double { return Xs[s * SPG_TILE + pc[q].s0 + off]; };
 
     // ---- prologue: pencil positions -3 .. 3 (faces 0, 1; zone 0)
-    double f0[PP], f1[PP], fn[PP][4];
+    // the face mass fluxes are requested two groups of four ahead of their use (they come from HBM)
+    double f0[PP], f1[PP], fn[PP][4], fnn[PP][4];
 #pragma unroll
     for (int q = 0; q < PP; ++q) {
         f0[q] = spg_ldg(fm + q * nthr, keep); f1[q] = spg_ldg(fm + q * nthr + NTHR, keep);
 #pragma unroll
         for (int e = 0; e < 4; ++e) fn[q][e] = spg_ldg(fm + q * nthr + (2 + e) * NTHR, keep);
+#pragma unroll
+        for (int e = 0; e < 4; ++e) fnn[q][e] = spg_ldg(fm + q * nthr + (6 + e) * NTHR, keep);
     }
 #pragma unroll
     for (int s = 0; s < G; ++s)
@@ -162,7 +166,8 @@ __device__ __forceinline__ void spg_sweep(const SpgPencil (&pc)[PP], const bool 
 #pragma unroll
             for (int e = 0; e < 4; ++e) {
                 fc[q][e] = fn[q][e];
-                if (it < 3 || e < 3) fn[q][e] = spg_ldg(fm + q * nthr + (4 * it + 2 + e) * NTHR, keep);
+                fn[q][e] = fnn[q][e];
+                if (it < 2 || (it == 2 && e < 3)) fnn[q][e] = spg_ldg(fm + q * nthr + (4 * it + 6 + e) * NTHR, keep);
             }
         const int p0 = 4 * it * sst;
 #pragma unroll
@@ -194,10 +199,13 @@ __device__ __forceinline__ void spg_sweep(const SpgPencil (&pc)[PP], const bool 
 // streaming phase: write out the n_out species from c_out0 (A and, fused, U_next) out of Ps, stage the
 // n_in species from c_in0 into Xs.  Rows of the tile are handled as 8 x 16-byte pieces: thread t takes
 // piece cp = t % 8 of rows t / 8 + (32 / PP) n (row = 16 k + j): every global access is a 16-byte vector.
-template <int G, int PP, int NR>
+// With HS (PP = 1 only) the 3-deep halos of all three directions are staged too, into
+// Hs[s][direction][n = 0..5][pencil id] (n < 3: positions -3..-1, n >= 3: positions 16..18).
+template <int G, int PP, int NR, bool HS>
 __device__ __forceinline__ void spg_stream(const Geom& g, const TileCoord& tc, const double* __restrict__ Ub,
                                            const double* __restrict__ rinv_b, double* __restrict__ Xs,
-                                           const double* __restrict__ Ps, double* __restrict__ A, const UpdArgs& up,
+                                           const double* __restrict__ Ps, double* __restrict__ Hs,
+                                           double* __restrict__ A, const UpdArgs& up,
                                            const int c_out0, const int n_out, const int c_in0, const int n_in)
 {
     const int ng = CST_NG;
@@ -223,6 +231,41 @@ __device__ __forceinline__ void spg_stream(const Geom& g, const TileCoord& tc, c
 #pragma unroll
             for (int s = 0; s < G; ++s)
                 if (s < n_in) { x[s * SPG_TILE] = u[s][n].x * ri[n].x; x[s * SPG_TILE + 1] = u[s][n].y * ri[n].y; }
+        }
+        if (HS) {
+            const long long zt0 = zt - 2 * cp;
+            // y halos (consumer pencil = 16 k + i) and z halos (consumer pencil = 16 j + i): 768 16-byte pieces each
+#pragma unroll
+            for (int m = 0; m < 3; ++m) {
+                const int idx = tid + NTHR * m, hp = idx & 7, q = (idx >> 3) & 15, n = idx >> 7;
+                const int off = n < 3 ? n - 3 : TILE - 3 + n;
+                const long long zy = zt0 + q * g.plane_g + (long long)off * g.ex + 2 * hp;
+                const long long zz = zt0 + off * g.plane_g + (long long)q * g.ex + 2 * hp;
+                const double2 ry = spg_ldg2(rinv_b + zy, keep), rz = spg_ldg2(rinv_b + zz, keep);
+#pragma unroll
+                for (int s = 0; s < G; ++s)
+                    if (s < n_in) {
+                        const double* Us = Ub + (long long)(c_in0 + s) * g.comp_g;
+                        const double2 uy = spg_ldg2(Us + zy), uz = spg_ldg2(Us + zz);
+                        double* h = Hs + s * SPG_HALO;
+                        *reinterpret_cast<double2*>(h + (6 + n) * NTHR + q * TILE + 2 * hp) = make_double2(uy.x * ry.x, uy.y * ry.y);
+                        *reinterpret_cast<double2*>(h + (12 + n) * NTHR + q * TILE + 2 * hp) = make_double2(uz.x * rz.x, uz.y * rz.y);
+                    }
+            }
+            // x halos of this thread's own x pencil (j = tid % 16, k = tid / 16): positions -3 | -2 -1 and 16 17 | 18
+            const long long zx = zt0 + (tid >> 4) * g.plane_g + (long long)(tid & 15) * g.ex;
+            const double rl = spg_ldg(rinv_b + zx - 3, keep), rh = spg_ldg(rinv_b + zx + TILE + 2, keep);
+            const double2 rl2 = spg_ldg2(rinv_b + zx - 2, keep), rh2 = spg_ldg2(rinv_b + zx + TILE, keep);
+#pragma unroll
+            for (int s = 0; s < G; ++s)
+                if (s < n_in) {
+                    const double* Us = Ub + (long long)(c_in0 + s) * g.comp_g;
+                    const double ul = Us[zx - 3], uh = Us[zx + TILE + 2];
+                    const double2 ul2 = spg_ldg2(Us + zx - 2), uh2 = spg_ldg2(Us + zx + TILE);
+                    double* h = Hs + s * SPG_HALO + tid;
+                    h[0] = ul * rl; h[NTHR] = ul2.x * rl2.x; h[2 * NTHR] = ul2.y * rl2.y;
+                    h[3 * NTHR] = uh2.x * rh2.x; h[4 * NTHR] = uh2.y * rh2.y; h[5 * NTHR] = uh * rh;
+                }
         }
     }
     if (n_out > 0) {
@@ -268,43 +311,53 @@ __device__ __forceinline__ void spg_stream(const Geom& g, const TileCoord& tc, c
 }
 
 // all species of one full tile, G at a time
-template <int G, int PP, int NR>
+template <int G, int PP, int NR, bool HS>
 __device__ __forceinline__ void spg_tile(const Geom& g, const TileCoord& tc, const double* __restrict__ Ub,
                                          const double* __restrict__ rinv_b, const double* __restrict__ fm_tile,
                                          double* __restrict__ A, const UpdArgs& up, double* __restrict__ sm)
 {
+    static_assert(!HS || PP == 1, "halo staging in shared memory is written for one pencil per thread");
     double* Xs = sm;                    // [G][SPG_TILE]  X of the tile core
     double* Ps = sm + G * SPG_TILE;     // [G][SPG_TILE]  A under construction
+    double* Hs = sm + 2 * G * SPG_TILE; // [G][SPG_HALO]  halo X values (HS only)
     const int tid = threadIdx.x, nthr = NTHR / PP;
     int c_prev = 0, n_prev = 0;
 #pragma unroll 1
     for (int s0 = 0; s0 < g.nspec; s0 += G) {
         const int n_in = min(G, g.nspec - s0), c_in = 5 + s0;
         __syncthreads();                                // z sweep of the previous group done
-        spg_stream<G, PP, NR>(g, tc, Ub, rinv_b, Xs, Ps, A, up, c_prev, n_prev, c_in, n_in);
-        // halo operands of the x sweep (products formed after the barrier, when the loads have landed)
+        spg_stream<G, PP, NR, HS>(g, tc, Ub, rinv_b, Xs, Ps, Hs, A, up, c_prev, n_prev, c_in, n_in);
         SpgHaloRaw<G, PP> hr;
         SpgPencil pc[PP];
 #pragma unroll
         for (int q = 0; q < PP; ++q) pc[q] = spg_pencil(g, tc, 0, tid + q * nthr);
-        spg_halo_load<G, PP>(g, Ub, rinv_b, pc, c_in, n_in, hr);
+        // without HS: halo operands of the x sweep (products formed after the barrier, when the loads have landed)
+        if (!HS) spg_halo_load<G, PP>(g, Ub, rinv_b, pc, c_in, n_in, hr);
         __syncthreads();
 #pragma unroll 1
         for (int d = 0; d < 3; ++d) {
             double hx[G][PP][6];
-#pragma unroll
-            for (int s = 0; s < G; ++s)
-#pragma unroll
-                for (int q = 0; q < PP; ++q)
-#pragma unroll
-                    for (int n = 0; n < 6; ++n) hx[s][q][n] = hr.u[s][q][n] * hr.r[q][n];
             SpgPencil pcd[PP];
 #pragma unroll
             for (int q = 0; q < PP; ++q) pcd[q] = pc[q];
-            if (d < 2) {                                // operands of the next sweep: in flight during this one
+            if (HS) {
 #pragma unroll
-                for (int q = 0; q < PP; ++q) pc[q] = spg_pencil(g, tc, d + 1, tid + q * nthr);
-                spg_halo_load<G, PP>(g, Ub, rinv_b, pc, c_in, n_in, hr);
+                for (int s = 0; s < G; ++s)
+#pragma unroll
+                    for (int n = 0; n < 6; ++n) hx[s][0][n] = Hs[s * SPG_HALO + (d * 6 + n) * NTHR + tid];
+                if (d < 2) pc[0] = spg_pencil(g, tc, d + 1, tid);
+            } else {
+#pragma unroll
+                for (int s = 0; s < G; ++s)
+#pragma unroll
+                    for (int q = 0; q < PP; ++q)
+#pragma unroll
+                        for (int n = 0; n < 6; ++n) hx[s][q][n] = hr.u[s][q][n] * hr.r[q][n];
+                if (d < 2) {                            // operands of the next sweep: in flight during this one
+#pragma unroll
+                    for (int q = 0; q < PP; ++q) pc[q] = spg_pencil(g, tc, d + 1, tid + q * nthr);
+                    spg_halo_load<G, PP>(g, Ub, rinv_b, pc, c_in, n_in, hr);
+                }
             }
             spg_sweep<G, PP>(pcd, d == 0, Xs, Ps, fm_tile + (d * (TILE + 1)) * NTHR, hx);
             if (d < 2) __syncthreads();
@@ -312,5 +365,5 @@ __device__ __forceinline__ void spg_tile(const Geom& g, const TileCoord& tc, con
         c_prev = c_in; n_prev = n_in;
     }
     __syncthreads();
-    spg_stream<G, PP, NR>(g, tc, Ub, rinv_b, Xs, Ps, A, up, c_prev, n_prev, 0, 0);
+    spg_stream<G, PP, NR, HS>(g, tc, Ub, rinv_b, Xs, Ps, Hs, A, up, c_prev, n_prev, 0, 0);
 }
