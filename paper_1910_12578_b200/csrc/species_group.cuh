@@ -90,9 +90,9 @@ struct SpgHaloRaw {
 template <int G, int PP>
 __device__ __forceinline__ void spg_halo_load(const Geom& g, const double* __restrict__ Ub,
                                               const double* __restrict__ rinv_b, const SpgPencil (&pc)[PP],
-                                              const int c0, const int ng_, SpgHaloRaw<G, PP>& h)
+                                              const int c0, const int ng_, SpgHaloRaw<G, PP>& h,
+                                              const unsigned long long keep)
 {
-    const unsigned long long keep = spg_policy_keep();
 #pragma unroll
     for (int q = 0; q < PP; ++q)
 #pragma unroll
@@ -111,12 +111,11 @@ __device__ __forceinline__ void spg_halo_load(const Geom& g, const double* __res
 template <int G, int PP>
 __device__ __forceinline__ void spg_sweep(const SpgPencil (&pc)[PP], const bool first, const double* __restrict__ Xs,
                                           double* __restrict__ Ps, const double* __restrict__ fm_d,
-                                          const double (&hx)[G][PP][6])
+                                          const double (&hx)[G][PP][6], const unsigned long long keep)
 {
     const int sst = pc[0].sst;
     const double nrd = pc[0].nrd;
     const int nthr = NTHR / PP;
-    const unsigned long long keep = spg_policy_keep();
     PpmWindow w[G][PP];
     double Fprev[G][PP];
     const double* __restrict__ fm = fm_d + threadIdx.x;          // pencil q: + q * nthr
@@ -206,12 +205,13 @@ __device__ __forceinline__ void spg_stream(const Geom& g, const TileCoord& tc, c
                                            const double* __restrict__ rinv_b, double* __restrict__ Xs,
                                            const double* __restrict__ Ps, double* __restrict__ Hs,
                                            double* __restrict__ A, const UpdArgs& up,
-                                           const int c_out0, const int n_out, const int c_in0, const int n_in)
+                                           const int c_out0, const int n_out, const int c_in0, const int n_in,
+                                           const unsigned long long keep)
 {
     const int ng = CST_NG;
     const int tid = threadIdx.x, cp = tid & 7, r0 = tid >> 3;
     constexpr int RS = 32 / PP, NROW = 8 * PP;          // row stride and rows per thread
-    const unsigned long long keep = spg_policy_keep(), strm = spg_policy_stream();
+    const unsigned long long strm = spg_policy_stream();
     const long long zt = ((long long)(tc.k0 + ng) * g.ey + (tc.j0 + ng)) * g.ex + (tc.i0 + ng) + 2 * cp;
     if (n_in > 0) {
         // one batch: 1/rho and the G species of all eight rows
@@ -325,14 +325,16 @@ __device__ __forceinline__ void spg_tile(const Geom& g, const TileCoord& tc, con
 #pragma unroll 1
     for (int s0 = 0; s0 < g.nspec; s0 += G) {
         const int n_in = min(G, g.nspec - s0), c_in = 5 + s0;
+        // 1/rho and Fm of this tile stay in L2 (evict_last) until the last species, which demotes them
+        const unsigned long long keep = (s0 + G >= g.nspec) ? spg_policy_stream() : spg_policy_keep();
         __syncthreads();                                // z sweep of the previous group done
-        spg_stream<G, PP, NR, HS>(g, tc, Ub, rinv_b, Xs, Ps, Hs, A, up, c_prev, n_prev, c_in, n_in);
+        spg_stream<G, PP, NR, HS>(g, tc, Ub, rinv_b, Xs, Ps, Hs, A, up, c_prev, n_prev, c_in, n_in, keep);
         SpgHaloRaw<G, PP> hr;
         SpgPencil pc[PP];
 #pragma unroll
         for (int q = 0; q < PP; ++q) pc[q] = spg_pencil(g, tc, 0, tid + q * nthr);
         // without HS: halo operands of the x sweep (products formed after the barrier, when the loads have landed)
-        if (!HS) spg_halo_load<G, PP>(g, Ub, rinv_b, pc, c_in, n_in, hr);
+        if (!HS) spg_halo_load<G, PP>(g, Ub, rinv_b, pc, c_in, n_in, hr, keep);
         __syncthreads();
 #pragma unroll 1
         for (int d = 0; d < 3; ++d) {
@@ -356,14 +358,14 @@ __device__ __forceinline__ void spg_tile(const Geom& g, const TileCoord& tc, con
                 if (d < 2) {                            // operands of the next sweep: in flight during this one
 #pragma unroll
                     for (int q = 0; q < PP; ++q) pc[q] = spg_pencil(g, tc, d + 1, tid + q * nthr);
-                    spg_halo_load<G, PP>(g, Ub, rinv_b, pc, c_in, n_in, hr);
+                    spg_halo_load<G, PP>(g, Ub, rinv_b, pc, c_in, n_in, hr, keep);
                 }
             }
-            spg_sweep<G, PP>(pcd, d == 0, Xs, Ps, fm_tile + (d * (TILE + 1)) * NTHR, hx);
+            spg_sweep<G, PP>(pcd, d == 0, Xs, Ps, fm_tile + (d * (TILE + 1)) * NTHR, hx, keep);
             if (d < 2) __syncthreads();
         }
         c_prev = c_in; n_prev = n_in;
     }
     __syncthreads();
-    spg_stream<G, PP, NR, HS>(g, tc, Ub, rinv_b, Xs, Ps, Hs, A, up, c_prev, n_prev, 0, 0);
+    spg_stream<G, PP, NR, HS>(g, tc, Ub, rinv_b, Xs, Ps, Hs, A, up, c_prev, n_prev, 0, 0, spg_policy_stream());
 }
