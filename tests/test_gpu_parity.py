@@ -247,3 +247,103 @@ def test_step_host_matches_oracle():
     orc.sdc_update(cfg, Uno, Uo, dt, Ao, Ao, [Ao, Ao], [0.5 * dt, 0.5 * dt])
     assert comp_err(Ah, Ao).max() <= TOL
     assert comp_err(interior(cfg, Unh), interior(cfg, Uno)).max() <= TOL
+
+
+# ------------------------------------------------------------ fast-path dispatch and fall-backs --
+def _run_A_update(ctx, cfg, Ud, Aold_d, dt, off=0):
+    """fused call on (possibly misaligned) views: every array starts `off` doubles into its buffer."""
+    def view(t):
+        buf = torch.empty(t.numel() + 2, dtype=torch.float64, device=DEV)
+        v = buf[off:off + t.numel()].view(t.shape)
+        v.copy_(t)
+        return v
+    U, Ao = view(Ud), view(Aold_d)
+    A = view(torch.zeros(wl.a_shape(cfg), dtype=torch.float64, device=DEV))
+    Un = view(torch.full(wl.u_shape(cfg), 3.0, dtype=torch.float64, device=DEV))
+    ctx.advance_A_update(U, A, Un, dt, Ao, [Ao, A], [0.25 * dt, 0.75 * dt])
+    torch.cuda.synchronize()
+    return A.clone(), Un.clone()
+
+
+def test_misaligned_pointers_take_the_scalar_paths():
+    """Full 16^3 tiles with 16-byte aligned arrays run the vector fast paths; the same arrays shifted by
+    8 bytes must fall back (x_vec / vec_ok false) and give the same numbers bit for bit (A) / to rounding."""
+    cfg = small_cfg(n=(32, 16, 16), nspec=3, gamma=5 / 3)
+    ctx = Context(cfg)
+    Ud = dev(wl.random_state(cfg, 41)); ctx.fill_ghosts(Ud)
+    dt = ctx.cfl_dt(Ud, 0.5)
+    Aold = torch.randn(wl.a_shape(cfg), dtype=torch.float64, device=DEV)
+    A0, U0 = _run_A_update(ctx, cfg, Ud, Aold, dt, off=0)
+    A1, U1 = _run_A_update(ctx, cfg, Ud, Aold, dt, off=1)
+    Ao = orc.advance_A(cfg, Ud.cpu().numpy())
+    assert comp_err(A0.cpu().numpy(), Ao).max() <= TOL and comp_err(A1.cpu().numpy(), Ao).max() <= TOL
+    assert comp_err(U1.cpu().numpy(), U0.cpu().numpy()).max() <= 1e-14
+
+
+def test_mixed_full_and_ragged_tiles_with_species():
+    """boxes of 40 x 24 x 20: full 16^3 tiles (vector fast path inside the generic kernel) next to ragged ones."""
+    cfg = small_cfg(n=(40, 24, 20), nb=(1, 2, 1), nspec=4, gamma=1.4, bc=(0, 1, 2), grav=(0.0, 0.3, -0.2))
+    check_one_call_set(cfg, wl.random_state(cfg, 42))
+
+
+def test_many_quadrature_arrays_fall_back_to_unfused_calls():
+    """more than three distinct external arrays in Eq. (2): the fused call splits into A + update kernels."""
+    cfg = small_cfg(n=(16, 16, 16), nspec=2)
+    ctx = Context(cfg)
+    Ud = dev(wl.random_state(cfg, 43)); ctx.fill_ghosts(Ud)
+    Uo = Ud.cpu().numpy()
+    rng = np.random.default_rng(7)
+    Q = [rng.standard_normal(wl.a_shape(cfg)) for _ in range(4)]
+    Aold = rng.standard_normal(wl.a_shape(cfg))
+    w, dt = [0.1, -0.2, 0.3, 0.05], 1e-3
+    Ad = torch.empty(wl.a_shape(cfg), dtype=torch.float64, device=DEV)
+    Und = torch.full(wl.u_shape(cfg), 3.0, dtype=torch.float64, device=DEV)
+    ctx.advance_A_update(Ud, Ad, Und, dt, dev(Aold), [dev(q) for q in Q], w)
+    Ao = orc.advance_A(cfg, Uo)
+    Uno = np.full_like(Uo, 3.0)
+    orc.sdc_update(cfg, Uno, Uo, dt, Ao, Aold, Q, w)
+    assert comp_err(Ad.cpu().numpy(), Ao).max() <= TOL
+    assert comp_err(Und.cpu().numpy(), Uno).max() <= 10 * TOL
+
+
+def test_kernel_timing_aid():
+    cfg = small_cfg(n=(16, 16, 16), nspec=1)
+    ctx = Context(cfg)
+    Ud = dev(wl.random_state(cfg, 44)); ctx.fill_ghosts(Ud)
+    Ad = torch.empty(wl.a_shape(cfg), dtype=torch.float64, device=DEV)
+    with pytest.raises(CstError):
+        ctx.last_advance_ms()                         # timing never switched on
+    ctx.set_timing(True)
+    ctx.advance_A(Ud, Ad)
+    h, s = ctx.last_advance_ms()
+    assert h > 0 and s > 0
+
+
+def test_no_writes_outside_the_output_arrays():
+    """A, U_next and the workspace sit inside guard bands (compute-sanitizer is not available on the
+    GPU pool): after fill / advance / fused / update / cfl calls the bands must be untouched, for boxes
+    with full tiles, ragged tiles and a box lattice."""
+    G = 4096
+    for n, nb, ns in [((32, 16, 16), (2, 1, 1), 3), ((24, 20, 12), (1, 2, 1), 2), ((16, 16, 16), (1, 1, 1), 0)]:
+        cfg = wl.make_config(4, n=n, nb=nb, nspec=ns)
+        ctx = Context(cfg, workspace=None)
+
+        def guarded(numel, fill):
+            buf = torch.full((numel + 2 * G,), 7.25, dtype=torch.float64, device=DEV)
+            buf[G:G + numel] = fill
+            return buf, buf[G:G + numel]
+        nU, nA = int(np.prod(wl.u_shape(cfg))), int(np.prod(wl.a_shape(cfg)))
+        nW = (ctx.workspace_bytes() + 7) // 8
+        bU, U = guarded(nU, 0.0); bUn, Un = guarded(nU, 3.0); bA, A = guarded(nA, 0.0); bW, W = guarded(nW, 0.0)
+        U.view(wl.u_shape(cfg)).copy_(dev(wl.initial_state(cfg, ghost_value=0.0)))
+        ctx.set_workspace(W)
+        A0 = torch.zeros(nA, dtype=torch.float64, device=DEV)
+        ctx.fill_ghosts(U)
+        dt = ctx.cfl_dt(U, 0.5)
+        ctx.advance_A(U, A)
+        ctx.advance_A_update(U, A, Un, dt, A0, [A0, A], [0.5 * dt, 0.5 * dt])
+        ctx.sdc_update(Un, U, dt, A, A0, [A0], [dt])
+        torch.cuda.synchronize()
+        for b in (bU, bUn, bA, bW):
+            assert torch.all(b[:G] == 7.25) and torch.all(b[-G:] == 7.25), (n, nb, ns)
+        assert torch.isfinite(A).all() and torch.isfinite(Un).all()
