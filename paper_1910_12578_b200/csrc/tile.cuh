@@ -46,15 +46,32 @@ struct TileCoord {
     long long tile;           // global tile index
 };
 
-__device__ __forceinline__ TileCoord tile_coord(const Geom& g, const TileGeom& tg, long long tile)
+// blockIdx -> tile.  Tiles are numbered x-fastest inside a box (that number addresses the Fm workspace),
+// but a big box is WALKED brick by brick (8 x 8 x 4 tiles): the ~300 tiles that are resident on the GPU
+// at one time then form a compact brick whose halo reads hit in L2, instead of a one-tile-thick slab
+// whose z neighbours were evicted long ago.
+#define BRICK_X 8
+#define BRICK_Y 8
+#define BRICK_Z 4
+__device__ __forceinline__ TileCoord tile_coord(const Geom& g, const TileGeom& tg, long long blk)
 {
     TileCoord t;
-    t.tile = tile;
-    t.b = (int)(tile / tg.tiles_per_box);
-    int r = (int)(tile - (long long)t.b * tg.tiles_per_box);
-    const int tk = r / (tg.ntx * tg.nty);
-    r -= tk * tg.ntx * tg.nty;
-    const int tj = r / tg.ntx, ti = r - tj * tg.ntx;
+    t.b = (int)(blk / tg.tiles_per_box);
+    int r = (int)(blk - (long long)t.b * tg.tiles_per_box);
+    int ti, tj, tk;
+    if ((tg.ntx % BRICK_X == 0) && (tg.nty % BRICK_Y == 0) && (tg.ntz % BRICK_Z == 0)) {
+        const int per = BRICK_X * BRICK_Y * BRICK_Z;
+        const int brick = r / per, w = r - brick * per;
+        const int nbx = tg.ntx / BRICK_X, nby = tg.nty / BRICK_Y;
+        const int bz = brick / (nbx * nby), br = brick - bz * nbx * nby, by = br / nbx, bx = br - by * nbx;
+        const int wz = w / (BRICK_X * BRICK_Y), wr = w - wz * BRICK_X * BRICK_Y, wy = wr / BRICK_X, wx = wr - wy * BRICK_X;
+        ti = bx * BRICK_X + wx; tj = by * BRICK_Y + wy; tk = bz * BRICK_Z + wz;
+    } else {
+        tk = r / (tg.ntx * tg.nty);
+        r -= tk * tg.ntx * tg.nty;
+        tj = r / tg.ntx; ti = r - tj * tg.ntx;
+    }
+    t.tile = (long long)t.b * tg.tiles_per_box + ((long long)tk * tg.nty + tj) * tg.ntx + ti;
     t.i0 = ti * TILE; t.j0 = tj * TILE; t.k0 = tk * TILE;
     t.tx = min(TILE, g.nx - t.i0); t.ty = min(TILE, g.ny - t.j0); t.tz = min(TILE, g.nz - t.k0);
     return t;
