@@ -363,11 +363,9 @@ static int launch_hydro_nr(cst_ctx* ctx, const double* U, double* A, const UpdAr
     const Geom& g = ctx->g;
     const TileGeom tg = make_tile_geom(g);
     const size_t smem = 5ull * PART_COMP * sizeof(double);
-    static bool attr_set = false;
-    if (!attr_set) {
+    {   // per launch: the attribute belongs to the current device's instance of the kernel
         if (cudaFuncSetAttribute(k_advect_hydro<NR>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
             return CST_ECUDA;
-        attr_set = true;
     }
     double* rinv = ctx->ws;
     double* Fm = ctx->ws + ws_rinv_doubles(g);

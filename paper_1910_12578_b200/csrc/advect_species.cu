@@ -168,14 +168,12 @@ static int launch_species_nr(cst_ctx* ctx, const double* U, double* A, const Upd
     const TileGeom tg = make_tile_geom(g);
     const double* rinv = ctx->ws;
     const double* Fm = ctx->ws + ws_rinv_doubles(g);
-    static bool attr_set = false;
     const size_t smem_full = (2ull * SPG_G * SPG_TILE + (SPG_HS ? SPG_G * SPG_HALO : 0)) * sizeof(double);
     const size_t smem = 2ull * SP_TILE * sizeof(double);
-    if (!attr_set) {
+    {   // per launch: the attribute belongs to the current device's instance of the kernel
         if (cudaFuncSetAttribute(k_advect_species<NR>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess ||
             cudaFuncSetAttribute(k_advect_species_full<NR>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_full) != cudaSuccess)
             return CST_ECUDA;
-        attr_set = true;
     }
     // 16-byte vector accesses of the fast path need even row lengths (true for multiples of 16) and aligned bases
     const bool vec_ok = (g.nx % 2 == 0) &&
