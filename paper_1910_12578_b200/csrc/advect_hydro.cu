@@ -32,6 +32,13 @@ __device__ __forceinline__ void ldg256(const double* p, double v[4])
                  : "=d"(v[0]), "=d"(v[1]), "=d"(v[2]), "=d"(v[3]) : "l"(p));
 }
 
+__device__ __forceinline__ double ldg_now(const double* p)
+{   // a load the compiler may not sink to its first use: issued here, consumed much later
+    double v;
+    asm volatile("ld.global.nc.f64 %0, [%1];" : "=d"(v) : "l"(p));
+    return v;
+}
+
 struct HydroMarch {           // per-thread state of one pencil march
     PpmWindow w[5];
     double Fprev[5];
@@ -60,12 +67,12 @@ __device__ __forceinline__ void hydro_zone(const Geom& g, const TileCoord& tc, H
         ia0 = m.pA - up.A_base;                          // index of component 0 in the A-like arrays
         if (grav || NR >= 0) {
 #pragma unroll
-            for (int c = 0; c < 5; ++c) Um[c] = Ub[c * g.comp_g + m.zc];
+            for (int c = 0; c < 5; ++c) Um[c] = ldg_now(Ub + c * g.comp_g + m.zc);
         }
 #pragma unroll
         for (int c = 0; c < 5; ++c)
 #pragma unroll
-            for (int r = 0; r < NR; ++r) Pv[c][r] = up.P[r][ia0 + c * g.comp_a];
+            for (int r = 0; r < NR; ++r) Pv[c][r] = ldg_now(up.P[r] + ia0 + c * g.comp_a);
     }
     double W[5];
     const double r = cons_to_prim(g, Uc[0], Uc[1], Uc[2], Uc[3], Uc[4], W);
