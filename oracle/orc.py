@@ -167,3 +167,46 @@ def sdc_step_2nd(cfg, U, dt):
     U2 = U0.copy()
     sdc_update(cfg, U2, U0, dt, A0, A0, [A0, A1], w)
     return U2
+
+
+def lobatto_nodes_weights(M):
+    """Gauss-Lobatto nodes c_m on [0, 1] (M = 2: trapezoid, M = 3: Simpson) and the
+    node-to-node weights w[m][j] = integral over [c_m, c_{m+1}] of the Lagrange polynomial l_j
+    (SURVEY 8(c) Q17), here by integrating the interpolating polynomials numerically exactly."""
+    if M == 2:
+        c = np.array([0.0, 1.0])
+    elif M == 3:
+        c = np.array([0.0, 0.5, 1.0])
+    else:
+        raise ValueError("M must be 2 or 3")
+    w = np.zeros((M - 1, M))
+    for j in range(M):
+        y = np.zeros(M); y[j] = 1.0
+        P = np.polyint(np.polyfit(c, y, M - 1))
+        for m in range(M - 1):
+            w[m, j] = np.polyval(P, c[m + 1]) - np.polyval(P, c[m])
+    return c, w
+
+
+def sdc_step_nodes(cfg, U, dt, M=3, K=4, A_fn=None):
+    """One SDC step with M Gauss-Lobatto nodes and K iterations, R = 0 (Eq. (2)):
+      U^{m+1,(k+1)} = U^{m,(k+1)} + dt_m (A^{m,(k+1)} - A^{m,(k)}) + sum_j w_{m,j} A^{j,(k)},
+    every node starting from U^n.  Built only from oracle calls; A_fn(U_ghosted) -> interior A replaces
+    <A(U)> in the pins of the time integrator alone.  Returns the new ghosted state (ghosts stale)."""
+    c, wt = lobatto_nodes_weights(M)
+    A_of = A_fn if A_fn is not None else (lambda V: advance_A(cfg, V))
+    U0 = fill_ghosts(cfg, U.copy())
+    A0 = A_of(U0)
+    U_old, A_old = [U0] * M, [A0] * M
+    for k in range(K):
+        U_new, A_new = [U0], [A0]
+        for m in range(M - 1):
+            dtm = (c[m + 1] - c[m]) * dt
+            Un = U_new[m].copy()
+            sdc_update(cfg, Un, U_new[m], dtm, A_new[m], A_old[m], A_old, list(wt[m] * dt))
+            fill_ghosts(cfg, Un)
+            U_new.append(Un)
+            last = (k == K - 1) and (m == M - 2)
+            A_new.append(None if last else A_of(Un))
+        U_old, A_old = U_new, A_new
+    return U_old[M - 1]

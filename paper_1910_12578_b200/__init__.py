@@ -7,4 +7,4 @@ hand-written CUDA kernels for sm_100a behind the C ABI in include/cst.h.
   build     -- in-tree nvcc build of libcst.so
 """
 from . import workloads  # noqa: F401
-from .binding import Context, CstError, load, sdc_step_2nd  # noqa: F401
+from .binding import Context, CstError, load, sdc_step_2nd, sdc_step_nodes  # noqa: F401

@@ -347,3 +347,19 @@ def test_no_writes_outside_the_output_arrays():
         for b in (bU, bUn, bA, bW):
             assert torch.all(b[:G] == 7.25) and torch.all(b[-G:] == 7.25), (n, nb, ns)
         assert torch.isfinite(A).all() and torch.isfinite(Un).all()
+
+
+@pytest.mark.parametrize("M,K", [(3, 4), (2, 2)])
+def test_node_driver_matches_oracle(M, K):
+    """One SDC step with M Gauss-Lobatto nodes and K iterations (Simpson: 4th order in time),
+    library calls only, against the oracle's driver from the same state."""
+    from paper_1910_12578_b200 import sdc_step_nodes
+    cfg = small_cfg(n=(20, 16, 12), nb=(1, 1, 2), nspec=2, gamma=5 / 3, bc=(0, 1, 2), grav=(0.0, 0.0, -0.5))
+    U0 = wl.random_state(cfg, 61)
+    ctx = Context(cfg)
+    dt = 0.4 * orc.cfl_dt(cfg, orc.fill_ghosts(cfg, U0.copy()), 1.0)
+    Uo = orc.sdc_step_nodes(cfg, U0, dt, M=M, K=K)
+    Ug = dev(U0)
+    sdc_step_nodes(ctx, Ug, dt, M=M, K=K)
+    e = comp_err(interior(cfg, Ug.cpu().numpy()), interior(cfg, Uo))
+    assert e.max() <= TOL, e

@@ -328,3 +328,37 @@ def test_P15_smooth_pulse_second_order():
 def test_P15_smooth_pulse_second_order_fine():
     (e32, _, _), (e64, _, _) = pulse_error(32), pulse_error(64)
     assert e32 / e64 >= 3.5, (e32, e64)
+
+
+# --------------------------------------------------------------- SDC with M nodes, K iterations --
+def _linear_ode_error(M, K, dt, lam=-1.3):
+    """one step of U' = lam U with the oracle's node driver; returns |U_1 - exp(lam dt)|"""
+    cfg = small_cfg(n=(4, 4, 4))
+    U0 = np.ones(orc.u_shape(cfg))
+    A_fn = lambda V: lam * V[:, :, 4:-4, 4:-4, 4:-4].copy()
+    U1 = orc.sdc_step_nodes(cfg, U0, dt, M=M, K=K, A_fn=A_fn)
+    return abs(U1[0, 0, 5, 5, 5] - np.exp(lam * dt))
+
+
+@pytest.mark.parametrize("M,K,order", [(2, 1, 1), (2, 2, 2), (3, 1, 1), (3, 2, 2), (3, 3, 3), (3, 4, 4), (3, 6, 4)])
+def test_sdc_iterations_raise_the_order_up_to_the_quadrature(M, K, order):
+    """"each iteration ... increases the temporal order by one up to the order of the
+    integral"; L44: trapezoid -> 2nd order, Simpson -> 4th.  Local error of one step ~ dt^(order+1)."""
+    e1, e2 = _linear_ode_error(M, K, 0.2), _linear_ode_error(M, K, 0.1)
+    rate = np.log2(e1 / e2)
+    assert abs(rate - (order + 1)) < 0.25, (M, K, rate)
+
+
+def test_node_driver_with_two_nodes_is_the_second_order_step():
+    cfg = small_cfg(n=(8, 6, 5), nspec=1, gamma=5 / 3)
+    U = wl.random_state(cfg, 51)
+    dt = 0.3 * orc.cfl_dt(cfg, orc.fill_ghosts(cfg, U.copy()), 1.0)
+    a, b = orc.sdc_step_2nd(cfg, U, dt), orc.sdc_step_nodes(cfg, U, dt, M=2, K=2)
+    inner = (slice(None), slice(None), slice(4, -4), slice(4, -4), slice(4, -4))
+    assert np.abs(a[inner] - b[inner]).max() <= 1e-14 * np.abs(a[inner]).max()
+
+
+def test_lobatto_weights_closed_form():
+    c, w = orc.lobatto_nodes_weights(3)
+    assert np.allclose(w, np.array([[5, 8, -1], [-1, 8, 5]]) / 24.0, atol=1e-15)
+    assert np.allclose(orc.lobatto_nodes_weights(2)[1], [[0.5, 0.5]], atol=1e-15)
