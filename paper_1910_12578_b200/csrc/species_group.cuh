@@ -116,7 +116,7 @@ __device__ __forceinline__ void spg_sweep(const SpgPencil (&pc)[PP], const bool 
     const int sst = pc[0].sst;
     const double nrd = pc[0].nrd;
     const int nthr = NTHR / PP;
-    PpmWindow w[G][PP];
+    PpmWindow w[G][PP] = {};
     double Fprev[G][PP];
     const double* __restrict__ fm = fm_d + threadIdx.x;          // pencil q: + q * nthr
 
