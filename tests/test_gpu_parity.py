@@ -363,3 +363,67 @@ def test_node_driver_matches_oracle(M, K):
     sdc_step_nodes(ctx, Ug, dt, M=M, K=K)
     e = comp_err(interior(cfg, Ug.cpu().numpy()), interior(cfg, Uo))
     assert e.max() <= TOL, e
+
+
+# ------------------------------------------------------------ invariants on the GPU itself ------
+def _gpu_A(cfg, U_host):
+    ctx = Context(cfg)
+    Ud = dev(U_host); ctx.fill_ghosts(Ud)
+    Ad = torch.empty(wl.a_shape(cfg), dtype=torch.float64, device=DEV)
+    ctx.advance_A(Ud, Ad)
+    return Ad.cpu().numpy()
+
+
+def test_box_lattice_equals_single_box_bitwise_on_gpu():
+    """P13 on the GPU: A on 8 boxes of 16^3 (2 x 2 x 2 lattice) equals A on one 32^3 box bit for bit,
+    and so does A on 2 x 1 x 1 boxes of 16 x 32 x 32 (tile boundaries fall on box boundaries)."""
+    one = small_cfg(n=(32, 32, 32), nspec=2, gamma=5 / 3)
+    G = wl.to_global(one, wl.random_state(one, 71), ghosted=True)
+    ref = wl.to_global(one, _gpu_A(one, wl.from_global(one, G)))
+    for n, nb in [((16, 16, 16), (2, 2, 2)), ((16, 32, 32), (2, 1, 1))]:
+        cfg = small_cfg(n=n, nb=nb, nspec=2, gamma=5 / 3)
+        A = wl.to_global(cfg, _gpu_A(cfg, wl.from_global(cfg, G)))
+        assert np.array_equal(A, ref), (n, nb)
+
+
+def test_axis_permutation_and_mirror_on_gpu():
+    """P7 on the GPU: A(Pi U) = Pi A(U) for an x<->z permutation and an x mirror, to rounding."""
+    cfg = small_cfg(n=(16, 16, 16), nspec=2, gamma=1.4)
+    G = wl.to_global(cfg, wl.random_state(cfg, 72), ghosted=True)          # [N, z, y, x]
+    A = wl.to_global(cfg, _gpu_A(cfg, wl.from_global(cfg, G)))
+    # x <-> z: transpose the spatial axes and swap the x / z momenta
+    Gp = np.ascontiguousarray(G.transpose(0, 3, 2, 1)); Gp[[1, 3]] = Gp[[3, 1]]
+    Ap = wl.to_global(cfg, _gpu_A(cfg, wl.from_global(cfg, Gp)))
+    back = np.ascontiguousarray(Ap.transpose(0, 3, 2, 1)); back[[1, 3]] = back[[3, 1]]
+    assert comp_err(back[None], A[None]).max() <= 1e-13
+    # mirror in x: reverse x and negate the x momentum
+    Gm = np.ascontiguousarray(G[:, :, :, ::-1]); Gm[1] *= -1.0
+    Am = wl.to_global(cfg, _gpu_A(cfg, wl.from_global(cfg, Gm)))
+    backm = np.ascontiguousarray(Am[:, :, :, ::-1]); backm[1] *= -1.0
+    assert comp_err(backm[None], A[None]).max() <= 1e-13
+
+
+def test_uniform_species_follow_the_mass_flux_on_gpu():
+    """P8 on the GPU: X_k uniform in space => A[rho X_k] = X_k A[rho] to rounding."""
+    cfg = small_cfg(n=(16, 16, 16), nspec=3, gamma=5 / 3)
+    G = wl.to_global(cfg, wl.random_state(cfg, 73), ghosted=True)
+    X = np.array([0.2, 0.5, 0.3])
+    G[5:] = X[:, None, None, None] * G[0]
+    A = wl.to_global(cfg, _gpu_A(cfg, wl.from_global(cfg, G)))
+    for k in range(3):
+        assert np.abs(A[5 + k] - X[k] * A[0]).max() <= 1e-13 * np.abs(A[0]).max()
+
+
+@pytest.mark.parametrize("seed", range(8))
+def test_random_shapes_and_boundaries_against_oracle(seed):
+    """fuzz: random box sizes (full, ragged and mixed tiles), lattices, species counts, BC kinds, gravity"""
+    rng = np.random.default_rng([2024, seed])
+    n = tuple(int(x) for x in rng.choice([4, 7, 12, 16, 17, 20, 32, 33], size=3))
+    nb = tuple(int(x) for x in rng.choice([1, 1, 2, 3], size=3))
+    if np.prod(n) * np.prod(nb) > 40000:
+        nb = (1, 1, 1)
+    bc = tuple(int(x) for x in rng.integers(0, 3, size=3))
+    cfg = small_cfg(n=n, nb=nb, nspec=int(rng.choice([0, 1, 2, 5, 13])), gamma=float(rng.choice([1.4, 5 / 3])),
+                    bc=bc, grav=tuple(rng.choice([0.0, 0.0, -0.7, 0.4], size=3)))
+    res = check_one_call_set(cfg, wl.random_state(cfg, 100 + seed), quad=("simpson" if seed % 2 else "euler"))
+    print(n, nb, bc, cfg["nspec"], res)
