@@ -227,6 +227,7 @@ def main():
         dist.init_process_group("nccl", device_id=dev)
 
     ctx = Context(cfg)
+    ctx_sm_count = torch.cuda.get_device_properties(dev).multi_processor_count
     N, zones = wl.nvar(cfg), wl.nzones(cfg)
     ushape, ashape = wl.u_shape(cfg), wl.a_shape(cfg)
     ubytes, abytes = int(np.prod(ushape)) * 8, int(np.prod(ashape)) * 8
@@ -302,10 +303,10 @@ def main():
     ab = alg_bytes(cfg)
     peak, peak_src = measured_peaks()
     ms_hydro, ms_species = k_ms2[-1]
-    traffic = None
+    traffic, prof = None, {}
     try:
-        tj = json.load(open(os.path.join(ROOT, "profiles", "traffic.json")))
-        traffic = tj.get(f"configs[{cfg['index']}]", {}).get("k_advect_species_dram_bytes_per_launch")
+        prof = json.load(open(os.path.join(ROOT, "profiles", "traffic.json"))).get(f"configs[{cfg['index']}]", {})
+        traffic = prof.get("k_advect_species_dram_bytes_per_launch")
     except Exception:
         pass
     if N > 5:
@@ -320,6 +321,17 @@ def main():
                                   "advance_call_ms": k_ms,
                                   "advance_call_frac": ab["advance"] * zones / (k_ms * 1e-3) / 1e9 / peak},
                 "whole_step_frac": ab["step"] * zones / (ms_step * 1e-3) / 1e9 / peak}
+    # second roof (BASELINE.json north_star: "the slower of bytes/HBM bandwidth and FP64 flops/peak"): instruction issue.
+    # warp instructions per launch are ncu counts (profiles/traffic.json); peak = SMs x 4 schedulers x SM clock.
+    sm_hz = (clocks or {}).get("sm_mhz") or 1965.0
+    issue_peak = ctx_sm_count * 4 * sm_hz * 1e6
+    if prof.get("k_advect_species_warp_instr_per_launch"):
+        roofline["issue"] = {
+            "k_advect_species_issue_frac": prof["k_advect_species_warp_instr_per_launch"] / (ms_species * 1e-3) / issue_peak,
+            "k_advect_hydro_issue_frac": prof["k_advect_hydro_warp_instr_per_launch"] / (ms_hydro * 1e-3) / issue_peak,
+            "fp64_pipe_active_pct_ncu": {"species": prof.get("k_advect_species_fp64_pipe_active_pct_ncu"),
+                                         "hydro": prof.get("k_advect_hydro_fp64_pipe_active_pct_ncu")},
+            "note": "warp instructions per launch from ncu (profiles/r01_final.md); an FP64 instruction holds its pipe for 2 issue cycles"}
 
     # ---- end to end through the C ABI with HOST buffers (H2D + D2H inside the timed region) --
     e2e = None
