@@ -14,7 +14,7 @@
 //   spg_tile (species_group.cuh) -- full 16^3 tiles: one body of sweep code for the three directions,
 //                          looped march, 16-byte vector streaming phase, L2 residency hints;
 //   species_sweep (below) -- any tile extent (ragged edges of boxes whose sides are not multiples of 16).
-// Shared memory: 2 x 16*16*17 doubles = 69.6 KB per CTA; two CTAs (16 warps, 128 registers per
+// Shared memory of the fast path: 2 x 16^3 doubles = 64 KB per CTA; two CTAs (16 warps, 128 registers per
 // thread) share an SM and leave the L1 the rest of the 228 KB -- measured to matter.
 #include "sweep.cuh"
 #include "tile.cuh"

@@ -3,7 +3,8 @@
 // A CTA of 256 / PP threads owns one tile; every thread marches PP pencils of G species AT ONCE:
 // G x PP independent PPM windows in registers give each warp the instruction-level parallelism that
 // the FP64 pipe latency needs, the face mass fluxes Fm and 1/rho are fetched once per G species, and
-// 2 G x 16*16*17 doubles of shared memory per CTA leave room for several CTAs per SM, whose
+// 2 G x 16^3 doubles of shared memory per CTA (unpadded: zone (k, j, i) sits in column i ^ j of its row, which
+// keeps all three pencil orientations free of bank conflicts) leave room for several CTAs per SM, whose
 // streaming phases (stage the next group / write out the previous one) overlap the sweeps of the others.
 // The sweep is ONE body of code with the direction as a run-time argument (strides, bases), executed
 // three times, and its march is a loop over groups of four zones: the kernel stays in the
@@ -13,7 +14,14 @@
 #include "sweep.cuh"
 #include "tile.cuh"
 
+#ifndef SPG_SWZ
+#define SPG_SWZ 1          // 1: unpadded tile arrays (2 x 32 KB per species), zone (k, j, i) stored in column i ^ j
+#endif
+#if SPG_SWZ
+#define SPG_PITCH 16
+#else
 #define SPG_PITCH 17
+#endif
 #define SPG_TILE (TILE * TILE * SPG_PITCH)
 #define SPG_HALO (3 * 6 * NTHR)         // halo X values of one species: [direction][n][pencil id]
 
@@ -58,6 +66,7 @@ struct SpgPencil {
     long long z0;      // ghosted index (within a component of the box) of pencil position 0
     long long stride;  // ghosted stride along the pencil
     int s0, sst;       // shared-memory index of position 0 and stride along the pencil
+    int M, X;          // SPG_SWZ: column of position pos is ((pos & M) ^ X) on top of s0 + pos * sst
     double nrd;        // -1/delta_d
 };
 
@@ -69,15 +78,25 @@ __device__ __forceinline__ SpgPencil spg_pencil(const Geom& g, const TileCoord& 
     const long long zt = ((long long)(tc.k0 + ng) * g.ey + (tc.j0 + ng)) * g.ex + (tc.i0 + ng);
     if (d == 0) {           // (a, b) = (j, k)
         pc.z0 = zt + b * g.plane_g + (long long)a * g.ex; pc.stride = 1;
-        pc.s0 = (b * TILE + a) * SPG_PITCH; pc.sst = 1; pc.nrd = -g.rdx;
+        pc.s0 = (b * TILE + a) * SPG_PITCH; pc.sst = SPG_SWZ ? 0 : 1; pc.nrd = -g.rdx; pc.M = 15; pc.X = a;
     } else if (d == 1) {    // (a, b) = (i, k)
         pc.z0 = zt + b * g.plane_g + a; pc.stride = g.ex;
-        pc.s0 = (b * TILE) * SPG_PITCH + a; pc.sst = SPG_PITCH; pc.nrd = -g.rdy;
+        pc.s0 = (b * TILE) * SPG_PITCH + (SPG_SWZ ? 0 : a); pc.sst = SPG_PITCH; pc.nrd = -g.rdy; pc.M = 15; pc.X = a;
     } else {                // (a, b) = (i, j)
         pc.z0 = zt + (long long)b * g.ex + a; pc.stride = g.plane_g;
-        pc.s0 = b * SPG_PITCH + a; pc.sst = TILE * SPG_PITCH; pc.nrd = -g.rdz;
+        pc.s0 = b * SPG_PITCH + (SPG_SWZ ? 0 : a); pc.sst = TILE * SPG_PITCH; pc.nrd = -g.rdz; pc.M = 0; pc.X = a ^ b;
     }
     return pc;
+}
+
+// shared-memory offset of pencil position pos (0..15) inside a tile array
+__device__ __forceinline__ int spg_off(const SpgPencil& pc, const int pos)
+{
+#if SPG_SWZ
+    return pc.s0 + pos * pc.sst + ((pos & pc.M) ^ pc.X);
+#else
+    return pc.s0 + pos * pc.sst;
+#endif
 }
 
 // raw halo operands of the PP pencils: positions -3..-1 (n = 0..2) and 16..18 (n = 3..5)
@@ -113,7 +132,6 @@ __device__ __forceinline__ void spg_sweep(const SpgPencil (&pc)[PP], const bool 
                                           double* __restrict__ Ps, const double* __restrict__ fm_d,
                                           const double (&hx)[G][PP][6], const unsigned long long keep)
 {
-    const int sst = pc[0].sst;
     const double nrd = pc[0].nrd;
     const int nthr = NTHR / PP;
     PpmWindow w[G][PP] = {};
@@ -123,12 +141,12 @@ __device__ __forceinline__ void spg_sweep(const SpgPencil (&pc)[PP], const bool 
     auto face = [&](const int s, const int q, const double fmc) -> double {
         return fmc * (sign_bit(fmc) ? w[s][q].qm : w[s][q].qpL);
     };
-    auto zone = [&](const int s, const int q, const int qoff, const double dF) {
-        double* p = Ps + s * SPG_TILE + pc[q].s0 + qoff;
+    auto zone = [&](const int s, const int q, const int pos, const double dF) {
+        double* p = Ps + s * SPG_TILE + spg_off(pc[q], pos);
         const double old = first ? 0.0 : *p;
         *p = fma(dF, nrd, old);
     };
-    auto xval = [&](const int s, const int q, const int off) -> double { return Xs[s * SPG_TILE + pc[q].s0 + off]; };
+    auto xval = [&](const int s, const int q, const int pos) -> double { return Xs[s * SPG_TILE + spg_off(pc[q], pos)]; };
 
     // ---- prologue: pencil positions -3 .. 3 (faces 0, 1; zone 0)
     // the face mass fluxes are requested two groups of four ahead of their use (they come from HBM)
@@ -148,10 +166,10 @@ __device__ __forceinline__ void spg_sweep(const SpgPencil (&pc)[PP], const bool 
             PpmWindow& ww = w[s][q];
             ww.start(hx[s][q][0]); ww.warm1(hx[s][q][1]); ww.warm2(hx[s][q][2]);
             ww.warm3(xval(s, q, 0));
-            ww.push(xval(s, q, sst));
-            ww.push(xval(s, q, 2 * sst));
+            ww.push(xval(s, q, 1));
+            ww.push(xval(s, q, 2));
             const double F0 = face(s, q, f0[q]);
-            ww.push(xval(s, q, 3 * sst));
+            ww.push(xval(s, q, 3));
             const double F1 = face(s, q, f1[q]);
             zone(s, q, 0, F1 - F0);
             Fprev[s][q] = F1;
@@ -168,16 +186,16 @@ __device__ __forceinline__ void spg_sweep(const SpgPencil (&pc)[PP], const bool 
                 fn[q][e] = fnn[q][e];
                 if (it < 2 || (it == 2 && e < 3)) fnn[q][e] = spg_ldg(fm + q * nthr + (4 * it + 6 + e) * NTHR, keep);
             }
-        const int p0 = 4 * it * sst;
+        const int p0 = 4 * it;
 #pragma unroll
         for (int e = 0; e < 4; ++e)
 #pragma unroll
             for (int s = 0; s < G; ++s)
 #pragma unroll
                 for (int q = 0; q < PP; ++q) {
-                    w[s][q].push(xval(s, q, p0 + e * sst));
+                    w[s][q].push(xval(s, q, p0 + e));
                     const double F = face(s, q, fc[q][e]);
-                    zone(s, q, p0 + (e - 3) * sst, F - Fprev[s][q]);
+                    zone(s, q, p0 + e - 3, F - Fprev[s][q]);
                     Fprev[s][q] = F;
                 }
     }
@@ -190,7 +208,7 @@ __device__ __forceinline__ void spg_sweep(const SpgPencil (&pc)[PP], const bool 
             for (int q = 0; q < PP; ++q) {
                 w[s][q].push(hx[s][q][3 + e]);
                 const double F = face(s, q, fn[q][e]);
-                zone(s, q, (13 + e) * sst, F - Fprev[s][q]);
+                zone(s, q, 13 + e, F - Fprev[s][q]);
                 Fprev[s][q] = F;
             }
 }
@@ -227,10 +245,22 @@ __device__ __forceinline__ void spg_stream(const Geom& g, const TileCoord& tc, c
         }
 #pragma unroll
         for (int n = 0; n < NROW; ++n) {
-            double* x = Xs + (r0 + RS * n) * SPG_PITCH + 2 * cp;
+            const int row = r0 + RS * n;
+#if SPG_SWZ
+            double* x = Xs + row * SPG_PITCH + ((2 * cp) ^ (row & 14));
+            const bool odd = row & 1;                  // odd j: the two columns of the piece swap places
+#pragma unroll
+            for (int s = 0; s < G; ++s)
+                if (s < n_in) {
+                    const double vx = u[s][n].x * ri[n].x, vy = u[s][n].y * ri[n].y;
+                    *reinterpret_cast<double2*>(x + s * SPG_TILE) = odd ? make_double2(vy, vx) : make_double2(vx, vy);
+                }
+#else
+            double* x = Xs + row * SPG_PITCH + 2 * cp;
 #pragma unroll
             for (int s = 0; s < G; ++s)
                 if (s < n_in) { x[s * SPG_TILE] = u[s][n].x * ri[n].x; x[s * SPG_TILE + 1] = u[s][n].y * ri[n].y; }
+#endif
         }
         if (HS) {
             const long long zt0 = zt - 2 * cp;
@@ -293,8 +323,13 @@ __device__ __forceinline__ void spg_stream(const Geom& g, const TileCoord& tc, c
 #pragma unroll
                 for (int e = 0; e < 4; ++e) {
                     const int row = r0 + RS * (n0 + e), k = row >> 4, j = row & 15;
+#if SPG_SWZ
+                    const double2 raw = *reinterpret_cast<const double2*>(pss + row * SPG_PITCH + ((2 * cp) ^ (row & 14)));
+                    const double2 av = (row & 1) ? make_double2(raw.y, raw.x) : raw;
+#else
                     const double* x = pss + row * SPG_PITCH + 2 * cp;
                     const double2 av = make_double2(x[0], x[1]);
+#endif
                     if (NR >= 0) {
                         double2 acc = make_double2(fma(up.ca, av.x, um[e].x), fma(up.ca, av.y, um[e].y));
 #pragma unroll
@@ -316,6 +351,7 @@ __device__ __forceinline__ void spg_tile(const Geom& g, const TileCoord& tc, con
                                          const double* __restrict__ rinv_b, const double* __restrict__ fm_tile,
                                          double* __restrict__ A, const UpdArgs& up, double* __restrict__ sm)
 {
+    static_assert(!(HS && SPG_SWZ), "halo staging is not written for the swizzled layout");
     static_assert(!HS || PP == 1, "halo staging in shared memory is written for one pencil per thread");
     double* Xs = sm;                    // [G][SPG_TILE]  X of the tile core
     double* Ps = sm + G * SPG_TILE;     // [G][SPG_TILE]  A under construction
