@@ -260,7 +260,11 @@ def main():
     k_ev, k_ms2 = [], []
     ctx.set_timing(True)      # CUDA events around the two kernels of the advance, on this stream (cst.h)
 
+    step_ev = []
+
     def step(timed):
+        if timed:
+            step_ev.append(ev()); step_ev[-1].record()
         ctx.fill_ghosts(U)
         if timed:
             e0, e1 = ev(), ev()
@@ -295,6 +299,7 @@ def main():
     ms = allreduce_scalar(ms, "max", dev, world)
     clocks = sampler.stop(t_wall0, t_wall1) if sampler else None
     ms_step = ms / args.steps
+    per_step = [a.elapsed_time(b) for a, b in zip(step_ev, step_ev[1:] + [s1])]
     value = aggregate_value(zones, world, ms_step)
     k_ms = float(np.mean([a.elapsed_time(b) for a, b in k_ev]))
 
@@ -375,6 +380,7 @@ def main():
                            "l2": f"inputs larger than L2 ({(ubytes + 3 * abytes) / 1e9:.1f} GB touched per step)"
                                  if ubytes > 4e8 else "inputs fit in L2 (debug size)",
                            "parallelism": f"replicas x{world}" if world > 1 else "single GPU",
+                           "ms_per_step_best": float(min(per_step)), "ms_per_step_median": float(np.median(per_step)),
                            "debug_size_override": bool(args.n)},
                 "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline,
                 "cpu_baseline": cpu_baseline}
