@@ -101,6 +101,11 @@ int cst_advance_A_update(cst_ctx* ctx, const double* U_m, double* A_new_m, doubl
 int cst_cfl_dt_device(cst_ctx* ctx, const double* U, double cfl, double* dt_out_dev, void* stream);
 int cst_cfl_dt(cst_ctx* ctx, const double* U, double cfl, double* dt_out_host, void* stream);
 
+/* Optional input check (not on the hot path, which does not detect bad states): *n_bad_host (HOST pointer)
+ * receives the number of interior zones with a non-finite component, rho <= 0 or gamma-law pressure <= 0.
+ * Synchronises the stream. */
+int cst_validate(cst_ctx* ctx, const double* U, long long* n_bad_host, void* stream);
+
 /* Host-buffer convenience used for the end-to-end measurement: copies the interior+ghost array
  * U_host (HOST, layout of U) to the device buffers owned by the caller (U_dev, U_next_dev,
  * A_dev), runs fill_ghosts + advance_A_update (forward-Euler node update: A_old = A_quad = A_new)

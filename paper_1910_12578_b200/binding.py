@@ -12,7 +12,7 @@ LIB_PATH = os.path.join(_HERE, "libcst.so")
 MAX_QUAD = 4
 
 EXPORTS = ["cst_create", "cst_destroy", "cst_workspace_bytes", "cst_set_workspace", "cst_fill_ghosts", "cst_advance_A", "cst_sdc_update",
-           "cst_advance_A_update", "cst_cfl_dt_device", "cst_cfl_dt", "cst_step_host",
+           "cst_advance_A_update", "cst_cfl_dt_device", "cst_cfl_dt", "cst_validate", "cst_step_host",
            "cst_set_timing", "cst_last_advance_ms", "cst_launch_count", "cst_strerror", "cst_version"]
 
 
@@ -56,6 +56,7 @@ def load():
     lib.cst_advance_A_update.argtypes = [_vp, _vp, _vp, _vp, C.c_double, _vp, C.c_int, C.POINTER(_vp), _dp, _vp]
     lib.cst_cfl_dt_device.argtypes = [_vp, _vp, C.c_double, _vp, _vp]
     lib.cst_cfl_dt.argtypes = [_vp, _vp, C.c_double, _dp, _vp]
+    lib.cst_validate.argtypes = [_vp, _vp, C.POINTER(C.c_longlong), _vp]
     lib.cst_step_host.argtypes = [_vp, _vp, _vp, _vp, _vp, _vp, _vp, C.c_double, _vp]
     lib.cst_set_timing.argtypes = [_vp, C.c_int]
     lib.cst_last_advance_ms.argtypes = [_vp, _dp, _dp]
@@ -173,6 +174,11 @@ class Context:
         out = C.c_double(0.0)
         self._check(self.lib.cst_cfl_dt(self._h, _ptr(U), float(cfl), C.byref(out), _stream(stream)), "cst_cfl_dt")
         return out.value
+
+    def validate(self, U, stream=None):
+        n = C.c_longlong(0)
+        self._check(self.lib.cst_validate(self._h, _ptr(U), C.byref(n), _stream(stream)), "cst_validate")
+        return n.value
 
     def step_host(self, U_host, A_host, U_next_host, U_dev, U_next_dev, A_dev, dt_m, stream=None):
         self._check(self.lib.cst_step_host(self._h, _ptr(U_host), _ptr(A_host), _ptr(U_next_host), _ptr(U_dev),

@@ -159,6 +159,20 @@ extern "C" int cst_cfl_dt(cst_ctx* c, const double* U, double cfl, double* dt_ou
     return e == cudaSuccess ? CST_OK : cuda_fail(e);
 }
 
+extern "C" int cst_validate(cst_ctx* c, const double* U, long long* n_bad_host, void* stream)
+{
+    if (!c || !U || !n_bad_host) return CST_EINVAL;
+    cudaStream_t st = (cudaStream_t)stream;
+    int rc = check_launch(launch_validate(c, U, st));
+    if (rc) return rc;
+    unsigned long long n = 0;
+    cudaError_t e = cudaMemcpyAsync(&n, c->d_scratch + 2, sizeof(n), cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    if (e != cudaSuccess) return cuda_fail(e);
+    *n_bad_host = (long long)n;
+    return CST_OK;
+}
+
 extern "C" int cst_step_host(cst_ctx* c, const double* U_host, double* A_host, double* U_next_host,
                              double* U_dev, double* U_next_dev, double* A_dev, double dt_m, void* stream)
 {

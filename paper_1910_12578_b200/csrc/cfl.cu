@@ -63,6 +63,47 @@ k_cfl_max(Geom g, const double* __restrict__ U, double* scratch)
     }
 }
 
+// cst_validate: number of interior zones whose state is not usable (a non-finite component, rho <= 0 or p <= 0)
+__global__ void __launch_bounds__(256)
+k_validate(Geom g, const double* __restrict__ U, unsigned long long* count)
+{
+    const int ng = CST_NG;
+    const long long total = (long long)g.nbox * g.comp_a;
+    unsigned long long bad = 0;
+    for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < total;
+         t += (long long)gridDim.x * blockDim.x) {
+        const int i = (int)(t % g.nx);
+        const long long r1 = t / g.nx;
+        const int j = (int)(r1 % g.ny);
+        const long long r2 = r1 / g.ny;
+        const int k = (int)(r2 % g.nz);
+        const long long b = r2 / g.nz;
+        const long long z = b * g.box_g + ((long long)(k + ng) * g.ey + (j + ng)) * g.ex + (i + ng);
+        bool ok = true;
+        for (int c = 0; c < g.nvar; ++c) ok = ok && isfinite(U[z + c * g.comp_g]);
+        const double rho = U[z], mx = U[z + g.comp_g], my = U[z + 2 * g.comp_g], mz = U[z + 3 * g.comp_g];
+        const double p = g.gm1 * (U[z + 4 * g.comp_g] - 0.5 * (mx * mx + my * my + mz * mz) / rho);
+        ok = ok && (rho > 0.0) && (p > 0.0);
+        bad += ok ? 0 : 1;
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) bad += __shfl_xor_sync(0xffffffffu, bad, o);
+    if ((threadIdx.x & 31) == 0 && bad) atomicAdd(count, bad);
+}
+
+int launch_validate(cst_ctx* ctx, const double* U, cudaStream_t st)
+{
+    const Geom& g = ctx->g;
+    const long long total = (long long)g.nbox * g.comp_a;
+    long long nb = (total + 255) / 256;
+    const long long cap = (long long)ctx->sm_count * 16;
+    if (nb > cap) nb = cap;
+    k_cfl_reset<<<1, 1, 0, st>>>(ctx->d_scratch + 2);
+    k_validate<<<(unsigned)nb, 256, 0, st>>>(g, U, reinterpret_cast<unsigned long long*>(ctx->d_scratch + 2));
+    ctx->launches += 2;
+    return cudaGetLastError() == cudaSuccess ? CST_OK : CST_ECUDA;
+}
+
 __global__ void k_cfl_final(const double* scratch, double cfl, double* dt_out)
 {
     *dt_out = cfl / scratch[0];

@@ -427,3 +427,15 @@ def test_random_shapes_and_boundaries_against_oracle(seed):
                     bc=bc, grav=tuple(rng.choice([0.0, 0.0, -0.7, 0.4], size=3)))
     res = check_one_call_set(cfg, wl.random_state(cfg, 100 + seed), quad=("simpson" if seed % 2 else "euler"))
     print(n, nb, bc, cfg["nspec"], res)
+
+
+def test_validate_counts_unusable_zones():
+    cfg = small_cfg(n=(12, 10, 9), nb=(2, 1, 1), nspec=2)
+    ctx = Context(cfg)
+    Ud = dev(wl.random_state(cfg, 81)); ctx.fill_ghosts(Ud)
+    assert ctx.validate(Ud) == 0
+    Ud[0, 0, 5, 5, 5] = -1.0                  # negative density
+    Ud[1, 4, 6, 6, 6] = 0.0                   # zero total energy -> negative pressure
+    Ud[1, 6, 7, 7, 7] = float("nan")          # NaN in a species component
+    Ud[0, 0, 0, 0, 0] = float("nan")          # a ghost zone: not counted
+    assert ctx.validate(Ud) == 3
