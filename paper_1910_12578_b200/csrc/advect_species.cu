@@ -29,6 +29,9 @@
 #ifndef SPG_HS
 #define SPG_HS 0       // 1: stage the halos in shared memory too (needs SPG_PP == 1; costs the L1 its capacity)
 #endif
+#ifndef SPG_SPLIT
+#define SPG_SPLIT 3     // consecutive CTAs that share one tile (each takes a contiguous share of the species)
+#endif
 #define SPG_NT (NTHR / SPG_PP)
 #ifndef SPG_CTAS
 #define SPG_CTAS 2     // resident CTAs per SM the fast path is sized for (128 registers per thread)
@@ -126,7 +129,7 @@ k_advect_species(Geom g, TileGeom tg, const double* __restrict__ U, double* __re
     const double* fm_tile = Fm + tc.tile * 3LL * (TILE + 1) * NTHR;
     const int tid = threadIdx.x, ti = tid & (TILE - 1), tr = tid >> 4;   // tr = row group 0..15
     if (vec_ok && (tc.tx == TILE) && (tc.ty == TILE) && (tc.tz == TILE)) {
-        spg_tile<1, 1, NR, false>(g, tc, Ub, rinv_b, fm_tile, A, up, sm);
+        spg_tile<1, 1, NR, false>(g, tc, Ub, rinv_b, fm_tile, A, up, sm, 0, g.nspec);
         return;
     }
     // ghosted index of the tile zone (i = ti, j = tr, k = 0); row n of this thread is k = n
@@ -153,12 +156,16 @@ k_advect_species(Geom g, TileGeom tg, const double* __restrict__ U, double* __re
 template <int NR>
 __global__ void __launch_bounds__(SPG_NT, SPG_CTAS)
 k_advect_species_full(Geom g, TileGeom tg, const double* __restrict__ U, double* __restrict__ A,
-                      const double* __restrict__ rinv, const double* __restrict__ Fm, UpdArgs up)
+                      const double* __restrict__ rinv, const double* __restrict__ Fm, UpdArgs up, int split)
 {
+    // `split` consecutive CTAs share one tile, each taking a contiguous share of the species: the tiles that
+    // are in flight at one time (and with them the Fm / 1/rho working set that L2 has to keep) are split x fewer
     extern __shared__ double sm[];
-    const TileCoord tc = tile_coord(g, tg, blockIdx.x);
+    const int part = blockIdx.x % split;
+    const TileCoord tc = tile_coord(g, tg, blockIdx.x / split);
+    const int s_begin = (int)((long long)g.nspec * part / split), s_end = (int)((long long)g.nspec * (part + 1) / split);
     spg_tile<SPG_G, SPG_PP, NR, (SPG_HS != 0)>(g, tc, U + (long long)tc.b * g.box_g, rinv + (long long)tc.b * g.comp_g,
-                                Fm + tc.tile * 3LL * (TILE + 1) * NTHR, A, up, sm);
+                                Fm + tc.tile * 3LL * (TILE + 1) * NTHR, A, up, sm, s_begin, s_end);
 }
 
 template <int NR>
@@ -181,7 +188,10 @@ static int launch_species_nr(cst_ctx* ctx, const double* U, double* A, const Upd
                            (uintptr_t)up.P[1] | (uintptr_t)up.P[2] | (uintptr_t)rinv) & 15) == 0);
     const bool all_full = vec_ok && (g.nx % TILE == 0) && (g.ny % TILE == 0) && (g.nz % TILE == 0);
     if (all_full)
-        k_advect_species_full<NR><<<(unsigned)tg.ntiles, SPG_NT, smem_full, st>>>(g, tg, U, A, rinv, Fm, up);
+    {
+        const int split = g.nspec < SPG_SPLIT ? g.nspec : SPG_SPLIT;
+        k_advect_species_full<NR><<<(unsigned)(tg.ntiles * split), SPG_NT, smem_full, st>>>(g, tg, U, A, rinv, Fm, up, split);
+    }
     else
         k_advect_species<NR><<<(unsigned)tg.ntiles, NTHR, smem, st>>>(g, tg, U, A, rinv, Fm, up, vec_ok);
     ctx->launches++;

@@ -345,11 +345,12 @@ __device__ __forceinline__ void spg_stream(const Geom& g, const TileCoord& tc, c
     }
 }
 
-// all species of one full tile, G at a time
+// the species [s_begin, s_end) of one full tile, G at a time
 template <int G, int PP, int NR, bool HS>
 __device__ __forceinline__ void spg_tile(const Geom& g, const TileCoord& tc, const double* __restrict__ Ub,
                                          const double* __restrict__ rinv_b, const double* __restrict__ fm_tile,
-                                         double* __restrict__ A, const UpdArgs& up, double* __restrict__ sm)
+                                         double* __restrict__ A, const UpdArgs& up, double* __restrict__ sm,
+                                         const int s_begin, const int s_end)
 {
     static_assert(!(HS && SPG_SWZ), "halo staging is not written for the swizzled layout");
     static_assert(!HS || PP == 1, "halo staging in shared memory is written for one pencil per thread");
@@ -359,10 +360,10 @@ __device__ __forceinline__ void spg_tile(const Geom& g, const TileCoord& tc, con
     const int tid = threadIdx.x, nthr = NTHR / PP;
     int c_prev = 0, n_prev = 0;
 #pragma unroll 1
-    for (int s0 = 0; s0 < g.nspec; s0 += G) {
-        const int n_in = min(G, g.nspec - s0), c_in = 5 + s0;
+    for (int s0 = s_begin; s0 < s_end; s0 += G) {
+        const int n_in = min(G, s_end - s0), c_in = 5 + s0;
         // 1/rho and Fm of this tile stay in L2 (evict_last) until the last species, which demotes them
-        const unsigned long long keep = (s0 + G >= g.nspec) ? spg_policy_stream() : spg_policy_keep();
+        const unsigned long long keep = (s0 + G >= s_end) ? spg_policy_stream() : spg_policy_keep();
         __syncthreads();                                // z sweep of the previous group done
         spg_stream<G, PP, NR, HS>(g, tc, Ub, rinv_b, Xs, Ps, Hs, A, up, c_prev, n_prev, c_in, n_in, keep);
         SpgHaloRaw<G, PP> hr;
