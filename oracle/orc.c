@@ -25,7 +25,9 @@
  * permutation/mirror invariance (P7), species identity (P8), cubic edge
  * exactness (P9), limiter bounds (P10), hydrostatic residual order (P11),
  * Heun / Simpson (P12), box-lattice equivalence + brute-force ghost map (P13),
- * CFL closed form (P14), 2nd-order convergence (P15).
+ * CFL closed form (P14), 2nd-order convergence (P15); the M-node SDC driver of orc.py: order rises by one per
+ * iteration up to the order of the quadrature on U' = lambda U; tests/golden/oracle_tiny_case.txt
+ * freezes the arithmetic of this file (written by tests/golden/make_golden.py from the oracle only).
  * Unpinned by the paper itself (conventions only): HLLC wave-speed estimate,
  * CW84-vs-other limiter, method-of-lines-vs-CTU -- see DESIGN.md.
  *
