@@ -232,16 +232,24 @@ __device__ __forceinline__ void spg_stream(const Geom& g, const TileCoord& tc, c
     const unsigned long long strm = spg_policy_stream();
     const long long zt = ((long long)(tc.k0 + ng) * g.ey + (tc.j0 + ng)) * g.ex + (tc.i0 + ng) + 2 * cp;
     if (n_in > 0) {
-        // one batch: 1/rho and the G species of all eight rows
+        // one batch: 1/rho and the G species of all eight rows.  Rows r0 + RS n of this thread differ by RS / 16
+        // planes: running pointers, one 64-bit add per array and row
         double2 ri[NROW], u[G][NROW];
+        const long long zrow = zt + (long long)(r0 >> 4) * g.plane_g + (long long)(r0 & 15) * g.ex;
+        const long long zstep = (RS / 16) * g.plane_g;
+        const double* pr = rinv_b + zrow;
+        const double* pu[G];
+#pragma unroll
+        for (int s = 0; s < G; ++s) pu[s] = Ub + (long long)(c_in0 + s) * g.comp_g + zrow;
 #pragma unroll
         for (int n = 0; n < NROW; ++n) {
-            const int row = r0 + RS * n, k = row >> 4, j = row & 15;
-            const long long z = zt + k * g.plane_g + (long long)j * g.ex;
-            ri[n] = spg_ldg2(rinv_b + z, keep);
+            ri[n] = spg_ldg2(pr, keep);
+            pr += zstep;
 #pragma unroll
-            for (int s = 0; s < G; ++s)
-                if (s < n_in) u[s][n] = spg_ldg2(Ub + (long long)(c_in0 + s) * g.comp_g + z);
+            for (int s = 0; s < G; ++s) {
+                if (s < n_in) u[s][n] = spg_ldg2(pu[s]);
+                pu[s] += zstep;
+            }
         }
 #pragma unroll
         for (int n = 0; n < NROW; ++n) {
@@ -306,23 +314,32 @@ __device__ __forceinline__ void spg_stream(const Geom& g, const TileCoord& tc, c
             const long long ias = ia0 + (long long)(c_out0 + s) * g.comp_a;
             const long long ius = iu0 + (long long)(c_out0 + s) * g.comp_g;
             const double* __restrict__ pss = Ps + s * SPG_TILE;
-            // batches of four rows: every load of a batch is issued before its first store
+            // batches of four rows: every load of a batch is issued before its first store; running pointers
+            const long long arow = ias + ((long long)(r0 >> 4) * g.ny + (r0 & 15)) * g.nx;
+            const long long astep = (long long)(RS / 16) * g.ny * g.nx;
+            const long long urow = ius + (long long)(r0 >> 4) * g.plane_g + (long long)(r0 & 15) * g.ex;
+            const long long ustep = (RS / 16) * g.plane_g;
+            const double* pum = up.U_m + urow;
+            double* pun = up.U_next + urow;
+            double* pa = A + arow;
+            const double* pp[UPD_MAX_EXT];
+#pragma unroll
+            for (int r = 0; r < UPD_MAX_EXT; ++r) pp[r] = (r < NR) ? up.P[r] + arow : nullptr;
 #pragma unroll
             for (int n0 = 0; n0 < NROW; n0 += 4) {
                 double2 um[4], pv[4][UPD_MAX_EXT];
 #pragma unroll
                 for (int e = 0; e < 4; ++e) {
-                    const int row = r0 + RS * (n0 + e), k = row >> 4, j = row & 15;
                     if (NR >= 0) {
-                        um[e] = spg_ldg2(up.U_m + ius + k * g.plane_g + (long long)j * g.ex);
+                        um[e] = spg_ldg2(pum);
+                        pum += ustep;
 #pragma unroll
-                        for (int r = 0; r < NR; ++r)
-                            pv[e][r] = spg_ldg2(up.P[r] + ias + ((long long)k * g.ny + j) * g.nx, strm);
+                        for (int r = 0; r < NR; ++r) { pv[e][r] = spg_ldg2(pp[r], strm); pp[r] += astep; }
                     }
                 }
 #pragma unroll
                 for (int e = 0; e < 4; ++e) {
-                    const int row = r0 + RS * (n0 + e), k = row >> 4, j = row & 15;
+                    const int row = r0 + RS * (n0 + e);
 #if SPG_SWZ
                     const double2 raw = *reinterpret_cast<const double2*>(pss + row * SPG_PITCH + ((2 * cp) ^ (row & 14)));
                     const double2 av = (row & 1) ? make_double2(raw.y, raw.x) : raw;
@@ -336,9 +353,11 @@ __device__ __forceinline__ void spg_stream(const Geom& g, const TileCoord& tc, c
                         for (int r = 0; r < NR; ++r) {
                             acc.x = fma(up.c[r], pv[e][r].x, acc.x); acc.y = fma(up.c[r], pv[e][r].y, acc.y);
                         }
-                        spg_stg2(up.U_next + ius + k * g.plane_g + (long long)j * g.ex, acc, strm);
+                        spg_stg2(pun, acc, strm);
+                        pun += ustep;
                     }
-                    spg_stg2(A + ias + ((long long)k * g.ny + j) * g.nx, av, strm);
+                    spg_stg2(pa, av, strm);
+                    pa += astep;
                 }
             }
         }
