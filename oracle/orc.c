@@ -28,7 +28,11 @@
  * CFL closed form (P14), 2nd-order convergence (P15); the M-node SDC driver of orc.py: order rises by one per
  * iteration up to the order of the quadrature on U' = lambda U; tests/golden/oracle_tiny_case.txt
  * freezes the arithmetic of this file (written by tests/golden/make_golden.py from the oracle only).
- * Unpinned by the paper itself (conventions only): HLLC wave-speed estimate,
+ * Round 2 (tests/test_oracle_pins2.py): the shock branch of the wave-speed estimate (orc_wave_speeds fed the
+ * exact star pressure returns the exact shock speed: textbook Sod value and the Rankine-Hugoniot mass
+ * condition on random shocks), orc_hllc against the textbook HLLC written out on those speeds, and the
+ * interface floors of line_fluxes against a brute-force restatement with floors that bind.
+ * Unpinned by the paper itself (conventions only): the CHOICE of the PVRS wave-speed estimate,
  * CW84-vs-other limiter, method-of-lines-vs-CTU -- see DESIGN.md.
  *
  * Data layout: U[b][c][k][j][i] on ghosted extents
@@ -199,17 +203,38 @@ void orc_ppm_line(int n, const double *q, double *qm, double *qp)
  * (pin P6; Q7b):
  *   rho* = rho_K r,  (rho v)* = rho* (v with normal component -> S*),
  *   E*   = r [E_K + (S* - u_K)(rho_K S* + p_K/(S_K - u_K))]. */
+/* Wave-speed estimate of the HLLC solver (Q6; Toro ch. 10, pressure-based): given the two normal
+ * states and an estimate ps of the star pressure,
+ *   S_L = u_L - c_L q_L,  S_R = u_R + c_R q_R,  q_K = 1 if ps <= p_K (rarefaction)
+ *   else sqrt(1 + (gamma+1)/(2 gamma) (ps/p_K - 1)) (shock).
+ * Exported on its own so that the shock branch can be pinned: fed the EXACT star pressure it
+ * returns the exact shock speed (tests/test_oracle_pins.py, Sod: 1.752156). */
+void orc_wave_speeds(double gamma, double rL, double uL, double pL, double rR, double uR, double pR,
+                     double ps, double *SL_out, double *SR_out)
+{
+    const double cL = sqrt(gamma * pL / rL), cR = sqrt(gamma * pR / rR);
+    const double gfac = (gamma + 1.0) / (2.0 * gamma);
+    const double qL = (ps <= pL) ? 1.0 : sqrt(1.0 + gfac * (ps / pL - 1.0));
+    const double qR = (ps <= pR) ? 1.0 : sqrt(1.0 + gfac * (ps / pR - 1.0));
+    *SL_out = uL - cL * qL;
+    *SR_out = uR + cR * qR;
+}
+
+/* PVRS estimate of the star pressure (Toro (9.20)/(10.67)), floored at 0. */
+double orc_pvrs_pstar(double gamma, double rL, double uL, double pL, double rR, double uR, double pR)
+{
+    const double cL = sqrt(gamma * pL / rL), cR = sqrt(gamma * pR / rR);
+    const double ppv = 0.5 * (pL + pR) - 0.5 * (uR - uL) * (0.5 * (rL + rR)) * (0.5 * (cL + cR));
+    return ppv > 0.0 ? ppv : 0.0;
+}
+
 void orc_hllc(int N, int d, double gamma, const double *WL, const double *WR, double *F)
 {
     const double rL = WL[0], rR = WR[0], pL = WL[4], pR = WR[4];
     const double uL = WL[1 + d], uR = WR[1 + d];
-    const double cL = sqrt(gamma * pL / rL), cR = sqrt(gamma * pR / rR);
-    const double ppv = 0.5 * (pL + pR) - 0.5 * (uR - uL) * (0.5 * (rL + rR)) * (0.5 * (cL + cR));
-    const double ps = ppv > 0.0 ? ppv : 0.0;
-    const double gfac = (gamma + 1.0) / (2.0 * gamma);
-    const double qL = (ps <= pL) ? 1.0 : sqrt(1.0 + gfac * (ps / pL - 1.0));
-    const double qR = (ps <= pR) ? 1.0 : sqrt(1.0 + gfac * (ps / pR - 1.0));
-    const double SL = uL - cL * qL, SR = uR + cR * qR;
+    const double ps = orc_pvrs_pstar(gamma, rL, uL, pL, rR, uR, pR);
+    double SL, SR;
+    orc_wave_speeds(gamma, rL, uL, pL, rR, uR, pR, ps, &SL, &SR);
     const double Ss = (pR - pL + rL * uL * (SL - uL) - rR * uR * (SR - uR))
                     / (rL * (SL - uL) - rR * (SR - uR));
     const double *W; double SK;

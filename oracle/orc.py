@@ -40,6 +40,10 @@ def lib():
         _lib.orc_ppm_line.restype = None
         _lib.orc_hllc.argtypes = [C.c_int, C.c_int, C.c_double, _dp, _dp, _dp]
         _lib.orc_hllc.restype = None
+        _lib.orc_wave_speeds.argtypes = [C.c_double] * 8 + [_dp, _dp]
+        _lib.orc_wave_speeds.restype = None
+        _lib.orc_pvrs_pstar.argtypes = [C.c_double] * 7
+        _lib.orc_pvrs_pstar.restype = C.c_double
         _lib.orc_exact_riemann_star.argtypes = [C.c_double] * 7 + [_dp]
         _lib.orc_exact_riemann_sample.argtypes = [C.c_double] * 7 + [C.c_int, _dp, _dp, _dp, _dp]
         _lib.orc_num_threads.restype = C.c_int
@@ -132,6 +136,17 @@ def hllc(d, gamma, WL, WR):
     F = np.empty_like(WL)
     lib().orc_hllc(len(WL), d, gamma, _ptr(WL), _ptr(WR), _ptr(F))
     return F
+
+
+def wave_speeds(g, rL, uL, pL, rR, uR, pR, ps):
+    """(S_L, S_R) of the HLLC wave-speed estimate for a given star-pressure estimate ps."""
+    SL, SR = C.c_double(0.0), C.c_double(0.0)
+    lib().orc_wave_speeds(g, rL, uL, pL, rR, uR, pR, ps, C.byref(SL), C.byref(SR))
+    return SL.value, SR.value
+
+
+def pvrs_pstar(g, rL, uL, pL, rR, uR, pR):
+    return lib().orc_pvrs_pstar(g, rL, uL, pL, rR, uR, pR)
 
 
 def exact_riemann_star(g, rL, uL, pL, rR, uR, pR):
