@@ -20,6 +20,8 @@
  * owns only a few KB of device scratch (reduction cells).  No call allocates or frees device memory
  * after cst_create.
  * `stream` is a cudaStream_t passed as void* (NULL = legacy default stream).
+ * One context (and its workspace) serves ONE stream at a time: the reduction cells of cst_cfl_dt / cst_validate and
+ * the workspace are shared by all calls on the context; use one context per concurrent stream.
  *
  * ERRORS.  Every call returns 0 (CST_OK) or a negative code; nothing throws, aborts or prints.
  * Launches are asynchronous: a device fault surfaces as CST_ECUDA from the next synchronising
@@ -51,8 +53,11 @@ typedef struct {
 
 typedef struct cst_ctx cst_ctx;    /* opaque */
 
-/* Validates params (CST_EINVAL: NULL, ng != 4, n_d < ng, nspec out of range, non-positive
- * widths, gamma <= 1, bad or one-sided-periodic BC) and allocates the context's scratch. */
+/* Validates params (CST_EINVAL: NULL, ng != 4, n_d < ng, nspec out of range, more than 65535 boxes, non-positive
+ * widths, gamma <= 1, bad or one-sided-periodic BC) and allocates the context's scratch.
+ * Range of the state: the kernels form products such as gamma*p*rho and use reciprocal / square-root sequences
+ * without the special-case branches of the library routines, so rho and p (floors included) must stay within
+ * about [1e-140, 1e140]; outside it results are unspecified (the default floors 1e-200 never bind inside it). */
 int cst_create(const cst_params* params, cst_ctx** out);
 int cst_destroy(cst_ctx* ctx);
 
@@ -88,8 +93,9 @@ int cst_sdc_update(cst_ctx* ctx, double* U_next, const double* U_m, double dt_m,
 
 /* Fused S1-S5: A_new_m <- <A(U_m)> and the node update above with that A_new_m, in one pass over
  * U_m.  A_old_m or any A_quad[q] may be the A_new_m buffer itself (then they mean the value just
- * computed, as in the first SDC iteration where every node carries A(U^n)).  U_next must not
- * alias U_m (CST_EINVAL). */
+ * computed, as in the first SDC iteration where every node carries A(U^n)).  Neither output may be an
+ * input: U_next == U_m, U_next == A_old_m / A_quad[q], U_next == A_new_m or U_m == A_new_m give CST_EINVAL
+ * (partially overlapping buffers are not detected). */
 int cst_advance_A_update(cst_ctx* ctx, const double* U_m, double* A_new_m, double* U_next,
                          double dt_m, const double* A_old_m,
                          int nquad, const double* const* A_quad, const double* w_quad, void* stream);
@@ -120,6 +126,16 @@ int cst_step_host(cst_ctx* ctx, const double* U_host, double* A_host, double* U_
  * milliseconds (CST_EINVAL if timing was never switched on).  Off by default. */
 int cst_set_timing(cst_ctx* ctx, int on);
 int cst_last_advance_ms(cst_ctx* ctx, double* ms_hydro, double* ms_species);
+
+/* Test aids (tests/ only; not on the hot path).
+ * cst_debug_rcp_sqrt: rcp_dev[i], sqrt_dev[i] <- the kernels' own reciprocal / square-root sequences (MUFU seed +
+ *   Newton steps, csrc/hydro.cuh) of x_dev[i], i < n (DEVICE arrays), for an accuracy test in ulps.
+ * cst_debug_tile_map: map_dev (DEVICE, 8 ints per tile, cst_debug_tile_count() tiles) receives, for every CTA
+ *   index of the advance kernels' grid, (box, i0, j0, k0, tx, ty, tz, tile id) of the 16^3-zone tile it works on:
+ *   the map must be a bijection onto the tiles of all boxes. */
+int cst_debug_rcp_sqrt(const double* x_dev, double* rcp_dev, double* sqrt_dev, long long n, void* stream);
+long long cst_debug_tile_count(const cst_ctx* ctx);
+int cst_debug_tile_map(cst_ctx* ctx, int* map_dev, void* stream);
 
 /* Number of kernel launches issued through this context since creation (for bench accounting). */
 long long cst_launch_count(const cst_ctx* ctx);

@@ -10,31 +10,17 @@
 // pencil end come straight from global memory into the window.  The contributions to A accumulate
 // in a second shared array.
 //
-// Two bodies of the same arithmetic:
-//   spg_tile (species_group.cuh) -- full 16^3 tiles: one body of sweep code for the three directions,
-//                          looped march, 16-byte vector streaming phase, L2 residency hints;
-//   species_sweep (below) -- any tile extent (ragged edges of boxes whose sides are not multiples of 16).
-// Shared memory of the fast path: 2 x 16^3 doubles = 64 KB per CTA; two CTAs (16 warps, 128 registers per
-// thread) share an SM and leave the L1 the rest of the 228 KB -- measured to matter.
+// Two kernels, same arithmetic:
+//   k_advect_species_tma (species_tma.cuh) -- boxes made of full 16^3 tiles (every BASELINE config): TMA tile loads
+//                          double-buffered on mbarriers, L2 prefetches of every other operand stream, three CTAs
+//                          per tile (each a contiguous share of the species), two CTAs per SM;
+//   k_advect_species (below) -- any box shape (ragged tiles), unaligned arrays, or no TMA driver entry point.
 #include "sweep.cuh"
 #include "tile.cuh"
-#include "species_group.cuh"
+#include "species_tma.cuh"
 
-#ifndef SPG_G
-#define SPG_G 1        // species per pass of the full-tile fast path
-#endif
-#ifndef SPG_PP
-#define SPG_PP 1       // pencils per thread of the full-tile fast path (CTA = 256 / SPG_PP threads)
-#endif
-#ifndef SPG_HS
-#define SPG_HS 0       // 1: stage the halos in shared memory too (needs SPG_PP == 1; costs the L1 its capacity)
-#endif
-#ifndef SPG_SPLIT
-#define SPG_SPLIT 3     // consecutive CTAs that share one tile (each takes a contiguous share of the species)
-#endif
-#define SPG_NT (NTHR / SPG_PP)
-#ifndef SPG_CTAS
-#define SPG_CTAS 2     // resident CTAs per SM the fast path is sized for (128 registers per thread)
+#ifndef SPT_SPLIT
+#define SPT_SPLIT 3     // consecutive CTAs that share one tile (each takes a contiguous share of the species)
 #endif
 
 #define SP_PITCH 17
@@ -117,7 +103,7 @@ __device__ __forceinline__ void species_sweep(const Geom& g, const TileCoord& tc
 template <int NR>
 __global__ void __launch_bounds__(NTHR, 2)
 k_advect_species(Geom g, TileGeom tg, const double* __restrict__ U, double* __restrict__ A,
-                 const double* __restrict__ rinv, const double* __restrict__ Fm, UpdArgs up, bool vec_ok)
+                 const double* __restrict__ rinv, const double* __restrict__ Fm, UpdArgs up)
 {
     extern __shared__ double sm[];
     double* Xs = sm;                    // X_s = rho X_s / rho of the tile core
@@ -128,10 +114,6 @@ k_advect_species(Geom g, TileGeom tg, const double* __restrict__ U, double* __re
     const double* rinv_b = rinv + (long long)tc.b * g.comp_g;
     const double* fm_tile = Fm + tc.tile * 3LL * (TILE + 1) * NTHR;
     const int tid = threadIdx.x, ti = tid & (TILE - 1), tr = tid >> 4;   // tr = row group 0..15
-    if (vec_ok && (tc.tx == TILE) && (tc.ty == TILE) && (tc.tz == TILE)) {
-        spg_tile<1, 1, NR, false>(g, tc, Ub, rinv_b, fm_tile, A, up, sm, 0, g.nspec);
-        return;
-    }
     // ghosted index of the tile zone (i = ti, j = tr, k = 0); row n of this thread is k = n
     const long long zt = ((long long)(tc.k0 + ng) * g.ey + (tc.j0 + tr + ng)) * g.ex + (tc.i0 + ti + ng);
     for (int s = 0; s < g.nspec; ++s) {
@@ -152,20 +134,21 @@ k_advect_species(Geom g, TileGeom tg, const double* __restrict__ U, double* __re
     }
 }
 
-// every tile of every box is a full 16^3: CTAs of SPG_NT threads, SPG_PP pencils per thread (species_group.cuh)
+// every tile of every box is a full 16^3 (species_tma.cuh).  `split` consecutive CTAs share one tile, each taking a
+// contiguous share of the species: the tiles that are in flight at one time (and with them the Fm / 1/rho working
+// set that L2 has to keep) are split x fewer.
 template <int NR>
-__global__ void __launch_bounds__(SPG_NT, SPG_CTAS)
-k_advect_species_full(Geom g, TileGeom tg, const double* __restrict__ U, double* __restrict__ A,
-                      const double* __restrict__ rinv, const double* __restrict__ Fm, UpdArgs up, int split)
+__global__ void __launch_bounds__(NTHR, 2)
+k_advect_species_tma(const Geom g, const TileGeom tg, const __grid_constant__ SptMaps maps, const double* __restrict__ U,
+                     double* __restrict__ A, const double* __restrict__ rinv, const double* __restrict__ Fm,
+                     const UpdArgs up, const int split)
 {
-    // `split` consecutive CTAs share one tile, each taking a contiguous share of the species: the tiles that
-    // are in flight at one time (and with them the Fm / 1/rho working set that L2 has to keep) are split x fewer
-    extern __shared__ double sm[];
+    extern __shared__ __align__(128) double sm[];
     const int part = blockIdx.x % split;
     const TileCoord tc = tile_coord(g, tg, blockIdx.x / split);
     const int s_begin = (int)((long long)g.nspec * part / split), s_end = (int)((long long)g.nspec * (part + 1) / split);
-    spg_tile<SPG_G, SPG_PP, NR, (SPG_HS != 0)>(g, tc, U + (long long)tc.b * g.box_g, rinv + (long long)tc.b * g.comp_g,
-                                Fm + tc.tile * 3LL * (TILE + 1) * NTHR, A, up, sm, s_begin, s_end);
+    spt_tile<NR>(g, tc, maps, U + (long long)tc.b * g.box_g, rinv + (long long)tc.b * g.comp_g,
+                 Fm + tc.tile * 3LL * (TILE + 1) * NTHR, A, up, sm, s_begin, s_end);
 }
 
 template <int NR>
@@ -175,25 +158,32 @@ static int launch_species_nr(cst_ctx* ctx, const double* U, double* A, const Upd
     const TileGeom tg = make_tile_geom(g);
     const double* rinv = ctx->ws;
     const double* Fm = ctx->ws + ws_rinv_doubles(g);
-    const size_t smem_full = (2ull * SPG_G * SPG_TILE + (SPG_HS ? SPG_G * SPG_HALO : 0)) * sizeof(double);
-    const size_t smem = 2ull * SP_TILE * sizeof(double);
-    {   // per launch: the attribute belongs to the current device's instance of the kernel
-        if (cudaFuncSetAttribute(k_advect_species<NR>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess ||
-            cudaFuncSetAttribute(k_advect_species_full<NR>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_full) != cudaSuccess)
-            return CST_ECUDA;
-    }
-    // 16-byte vector accesses of the fast path need even row lengths (true for multiples of 16) and aligned bases
-    const bool vec_ok = (g.nx % 2 == 0) &&
-                        ((((uintptr_t)U | (uintptr_t)A | (uintptr_t)up.U_next | (uintptr_t)up.P[0] |
+    // 16-byte vector accesses and the tensor maps of the fast path need even rows (true for multiples of 16) and aligned bases
+    const bool vec_ok = ((((uintptr_t)U | (uintptr_t)A | (uintptr_t)up.U_next | (uintptr_t)up.P[0] |
                            (uintptr_t)up.P[1] | (uintptr_t)up.P[2] | (uintptr_t)rinv) & 15) == 0);
     const bool all_full = vec_ok && (g.nx % TILE == 0) && (g.ny % TILE == 0) && (g.nz % TILE == 0);
-    if (all_full)
-    {
-        const int split = g.nspec < SPG_SPLIT ? g.nspec : SPG_SPLIT;
-        k_advect_species_full<NR><<<(unsigned)(tg.ntiles * split), SPG_NT, smem_full, st>>>(g, tg, U, A, rinv, Fm, up, split);
+    bool tma = all_full;
+    SptMaps maps;
+    if (tma) {
+        const unsigned long long nbv = (unsigned long long)g.nbox * g.nvar;
+        tma = tma_encode_3d_f64(&maps.u, U, g.ex, g.ey, nbv * g.ez, SPT_PITCH, TILE, TILE) &&
+              tma_encode_3d_f64(&maps.r, rinv, g.ex, g.ey, (unsigned long long)g.nbox * g.ez, 24, 22, 22);
+        for (int r = 0; r < UPD_MAX_EXT; ++r)
+            maps.p[r] = maps.u;                               // unused slots: any valid map
+        for (int r = 0; tma && r < NR; ++r)
+            tma = tma_encode_3d_f64(&maps.p[r], up.P[r], g.nx, g.ny, nbv * g.nz, TILE, TILE, TILE);
     }
-    else
-        k_advect_species<NR><<<(unsigned)tg.ntiles, NTHR, smem, st>>>(g, tg, U, A, rinv, Fm, up, vec_ok);
+    if (tma) {
+        if (cudaFuncSetAttribute(k_advect_species_tma<NR>, cudaFuncAttributeMaxDynamicSharedMemorySize, SPT_SMEM) != cudaSuccess)
+            return CST_ECUDA;
+        const int split = g.nspec < SPT_SPLIT ? g.nspec : SPT_SPLIT;
+        k_advect_species_tma<NR><<<(unsigned)(tg.ntiles * split), NTHR, SPT_SMEM, st>>>(g, tg, maps, U, A, rinv, Fm, up, split);
+    } else {
+        const size_t smem = 2ull * SP_TILE * sizeof(double);
+        if (cudaFuncSetAttribute(k_advect_species<NR>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
+            return CST_ECUDA;
+        k_advect_species<NR><<<(unsigned)tg.ntiles, NTHR, smem, st>>>(g, tg, U, A, rinv, Fm, up);
+    }
     ctx->launches++;
     return cudaGetLastError() == cudaSuccess ? CST_OK : CST_ECUDA;
 }

@@ -139,6 +139,16 @@ extern "C" int cst_advance_A_update(cst_ctx* c, const double* U_m, double* A_new
     QuadArgs q;
     int rc = make_quad(nquad, A_quad, w_quad, q);
     if (rc) return rc;
+    // the outputs are written while the inputs are still being read through read-only loads: no output may be
+    // an input (A_old_m / A_quad[q] == A_new_m is the documented exception: it means "the value just computed")
+    const void* in[2 + CST_MAX_QUAD] = { U_m, A_old_m };
+    for (int n = 0; n < nquad; ++n) in[2 + n] = q.A[n];
+    for (int n = 0; n < 2 + nquad; ++n) {
+        if (in[n] == (const void*)U_next) return CST_EINVAL;
+        if (n != 0 && in[n] == (const void*)A_new_m) continue;
+        if (in[n] == (const void*)A_new_m) return CST_EINVAL;
+    }
+    if ((const void*)U_next == (const void*)A_new_m) return CST_EINVAL;
     return check_launch(launch_advance_A(c, U_m, A_new_m, U_next, dt_m, A_old_m, q, true, (cudaStream_t)stream));
 }
 
@@ -201,9 +211,14 @@ extern "C" int cst_step_host(cst_ctx* c, const double* U_host, double* A_host, d
 extern "C" int cst_set_timing(cst_ctx* c, int on)
 {
     if (!c) return CST_EINVAL;
-    if (on && !c->ev[0])
+    if (on && !c->ev[0]) {
         for (int n = 0; n < 3; ++n)
-            if (cudaEventCreate(&c->ev[n]) != cudaSuccess) return cuda_fail(cudaGetLastError());
+            if (cudaEventCreate(&c->ev[n]) != cudaSuccess) {
+                const int rc = cuda_fail(cudaGetLastError());
+                for (int m = 0; m < 3; ++m) { if (c->ev[m]) cudaEventDestroy(c->ev[m]); c->ev[m] = nullptr; }
+                return rc;
+            }
+    }
     c->timing = on ? 1 : 0;
     return CST_OK;
 }
@@ -218,6 +233,20 @@ extern "C" int cst_last_advance_ms(cst_ctx* c, double* ms_hydro, double* ms_spec
     if (e != cudaSuccess) return cuda_fail(e);
     *ms_hydro = a; *ms_species = b;
     return CST_OK;
+}
+
+extern "C" int cst_debug_rcp_sqrt(const double* x_dev, double* rcp_dev, double* sqrt_dev, long long n, void* stream)
+{
+    if (!x_dev || !rcp_dev || !sqrt_dev || n < 0) return CST_EINVAL;
+    return check_launch(launch_debug_rcp_sqrt(x_dev, rcp_dev, sqrt_dev, n, (cudaStream_t)stream));
+}
+
+extern "C" long long cst_debug_tile_count(const cst_ctx* c) { return c ? debug_tile_count(c->g) : -1; }
+
+extern "C" int cst_debug_tile_map(cst_ctx* c, int* map_dev, void* stream)
+{
+    if (!c || !map_dev) return CST_EINVAL;
+    return check_launch(launch_debug_tile_map(c, map_dev, (cudaStream_t)stream));
 }
 
 extern "C" long long cst_launch_count(const cst_ctx* c) { return c ? c->launches : -1; }

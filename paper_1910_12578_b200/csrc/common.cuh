@@ -64,3 +64,6 @@ int launch_sdc_update(cst_ctx*, double* U_next, const double* U_m, double dt_m,
                       const double* A_new_m, const double* A_old_m, const QuadArgs& q, cudaStream_t);
 int launch_cfl(cst_ctx*, const double* U, double cfl, double* dt_out_dev, cudaStream_t);
 int launch_validate(cst_ctx*, const double* U, cudaStream_t);   // count left in d_scratch[2]
+int launch_debug_rcp_sqrt(const double* x, double* r, double* s, long long n, cudaStream_t);
+long long debug_tile_count(const Geom& g);
+int launch_debug_tile_map(cst_ctx*, int* out, cudaStream_t);

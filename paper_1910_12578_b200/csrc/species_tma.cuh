@@ -1,0 +1,357 @@
+// species_tma.cuh -- fast path of the species kernel for boxes made of full 16^3 tiles (k_advect_species_tma).
+//
+// One CTA (256 threads) works on one 16^3 tile and a contiguous share of the species; two CTAs share an SM.  Per species:
+//   * rho X of the tile core arrives by ONE tensor-map (TMA) tile load -- issued a whole species pass earlier, double
+//     buffered, completing on an mbarrier -- so no compute warp ever waits for HBM on it;
+//   * the face mass fluxes Fm, 1/rho and the fused update's operands (A_old arrays) are pulled into L2 by bulk / tensor
+//     prefetches one pass ahead of the loads that use them;
+//   * X = rho X / rho is formed in place, then three sweeps (x, y, z), one pencil per thread with the PPM window in
+//     registers (sweep.cuh), accumulate -div F into the partial-sum tile; the next pass writes A (and U_next) out.
+// Shared-memory tiles are dense rows of 18 doubles (144 bytes: the TMA box is 18 zones wide): every access of every
+// sweep is "pencil base + immediate", rows stay 16-byte aligned, the x sweep reads and writes PAIRS of zones (16-byte
+// accesses: eight threads of a quarter warp hit eight different 16-byte bank groups because 9 j mod 8 is a permutation),
+// and the y / z sweeps touch 16 consecutive doubles per half warp -- no bank conflicts, no swizzle arithmetic.
+// Same arithmetic, zone for zone, as species_sweep (advect_species.cu) and as the oracle's S1-S5.
+#pragma once
+#include "sweep.cuh"
+#include "tile.cuh"
+#include "tma.cuh"
+
+#define SPT_PITCH 18
+#define SPT_PLANE (TILE * SPT_PITCH)          // 288 doubles
+#define SPT_TILE (TILE * SPT_PLANE)           // 4608 doubles
+#define SPT_TILE_BYTES (SPT_TILE * 8)         // 36864 = the TMA box 18 x 16 x 16
+#define SPT_SMEM (3 * SPT_TILE_BYTES + 128)   // X[2], P, two mbarriers
+
+struct SptMaps {             // tensor maps of one call (host-encoded, passed as a __grid_constant__ kernel parameter)
+    CUtensorMap u;           // U as [nbox*nvar*ez][ey][ex], box 18 x 16 x 16: the tile-core load
+    CUtensorMap r;           // 1/rho workspace as [nbox*ez][ey][ex], box 24 x 22 x 22: L2 prefetch of the tile's star
+    CUtensorMap p[UPD_MAX_EXT];   // external arrays of the fused update as [nbox*nvar*nz][ny][nx], box 16^3: L2 prefetch
+};
+
+__device__ __forceinline__ unsigned long long spt_policy_keep()
+{
+    unsigned long long p;
+    asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(p));
+    return p;
+}
+__device__ __forceinline__ unsigned long long spt_policy_stream()
+{
+    unsigned long long p;
+    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
+    return p;
+}
+__device__ __forceinline__ double spt_ldg(const double* a, unsigned long long pol)
+{
+    double v;
+    asm volatile("ld.global.nc.L2::cache_hint.f64 %0, [%1], %2;" : "=d"(v) : "l"(a), "l"(pol));
+    return v;
+}
+__device__ __forceinline__ double2 spt_ldg2(const double* a, unsigned long long pol)
+{
+    double2 v;
+    asm volatile("ld.global.nc.L2::cache_hint.v2.f64 {%0,%1}, [%2], %3;" : "=d"(v.x), "=d"(v.y) : "l"(a), "l"(pol));
+    return v;
+}
+__device__ __forceinline__ double2 spt_ldg2(const double* a)
+{
+    double2 v;
+    asm volatile("ld.global.nc.v2.f64 {%0,%1}, [%2];" : "=d"(v.x), "=d"(v.y) : "l"(a));
+    return v;
+}
+__device__ __forceinline__ void spt_stg2(double* a, double2 v, unsigned long long pol)
+{
+    asm volatile("st.global.L2::cache_hint.v2.f64 [%0], {%1,%2}, %3;" :: "l"(a), "d"(v.x), "d"(v.y), "l"(pol) : "memory");
+}
+
+// pencil of this thread in direction D: (a, b) = (tid % 16, tid / 16) = (j, k) | (i, k) | (i, j)
+template <int D> struct SptDir { static constexpr int SST = (D == 0) ? 1 : (D == 1) ? SPT_PITCH : SPT_PLANE; };
+
+template <int D>
+__device__ __forceinline__ int spt_sbase(const int a, const int b)
+{   // shared-memory index (doubles) of pencil position 0
+    return (D == 0) ? (b * TILE + a) * SPT_PITCH : (D == 1) ? b * SPT_PLANE + a : b * SPT_PITCH + a;
+}
+
+struct SptHalo { double u[6], r[6]; };      // raw rho X and 1/rho at pencil positions -3..-1 (0..2) and 16..18 (3..5)
+
+// halo operands of this thread's pencil in direction d (run time), straight from global memory: requested one sweep
+// before they are used
+__device__ __forceinline__ void spt_halo_load(const Geom& g, const TileCoord& tc, const int d, const double* __restrict__ Us,
+                                              const double* __restrict__ rinv_b, SptHalo& h, const unsigned long long keep)
+{
+    const int ng = CST_NG, a = threadIdx.x & (TILE - 1), b = threadIdx.x >> 4;
+    const long long zt = ((long long)(tc.k0 + ng) * g.ey + (tc.j0 + ng)) * g.ex + (tc.i0 + ng);
+    long long z0, stride;
+    if (d == 0) { z0 = zt + b * g.plane_g + (long long)a * g.ex; stride = 1; }
+    else if (d == 1) { z0 = zt + b * g.plane_g + a; stride = g.ex; }
+    else { z0 = zt + (long long)b * g.ex + a; stride = g.plane_g; }
+#pragma unroll
+    for (int n = 0; n < 6; ++n) {
+        const long long z = z0 + (long long)(n < 3 ? n - 3 : TILE - 3 + n) * stride;
+        h.r[n] = spt_ldg(rinv_b + z, keep);
+        h.u[n] = Us[z];
+    }
+}
+
+__device__ __forceinline__ double spt_face(const PpmWindow& w, const double fmc)
+{   // F(rho X) = F(rho) * X(upwind side): the sign of the mass flux picks the side (Q8)
+    return fmc * (sign_bit(fmc) ? w.qm : w.qpL);
+}
+
+// face mass fluxes of one pencil: thread-private slots fm[f * NTHR], f = 0..16, requested two groups of four ahead
+struct SptFm {
+    double f0, f1, fn[4], fnn[4];
+    __device__ __forceinline__ void start(const double* __restrict__ fm, const unsigned long long keep)
+    {
+        f0 = spt_ldg(fm, keep); f1 = spt_ldg(fm + NTHR, keep);
+#pragma unroll
+        for (int e = 0; e < 4; ++e) fn[e] = spt_ldg(fm + (2 + e) * NTHR, keep);
+#pragma unroll
+        for (int e = 0; e < 4; ++e) fnn[e] = spt_ldg(fm + (6 + e) * NTHR, keep);
+    }
+    // at the top of loop iteration it (1..3): fc <- faces 4it-2 .. 4it+1, and the request for faces 4it+6 ..
+    __device__ __forceinline__ void advance(const double* __restrict__ fm, const int it, double (&fc)[4], const unsigned long long keep)
+    {
+#pragma unroll
+        for (int e = 0; e < 4; ++e) {
+            fc[e] = fn[e];
+            fn[e] = fnn[e];
+            if (it < 2 || (it == 2 && e < 3)) fnn[e] = spt_ldg(fm + (4 * it + 6 + e) * NTHR, keep);
+        }
+    }
+};
+
+// y or z sweep: X and P of pencil position p at Xp[p * SST], Pp[p * SST] (compile-time strides)
+template <int D>
+__device__ __forceinline__ void spt_sweep_yz(const double* __restrict__ Xp, double* __restrict__ Pp,
+                                             const double* __restrict__ fm, const double (&hx)[6], const double nrd,
+                                             const unsigned long long keep)
+{
+    constexpr int S = SptDir<D>::SST;
+    PpmWindow w;
+    SptFm q;
+    q.start(fm, keep);
+    w.start(hx[0]); w.warm1(hx[1]); w.warm2(hx[2]);
+    w.warm3(Xp[0]);
+    w.push(Xp[S]);
+    w.push(Xp[2 * S]);
+    const double F0 = spt_face(w, q.f0);
+    w.push(Xp[3 * S]);
+    double Fprev = spt_face(w, q.f1);
+    Pp[0] = fma(Fprev - F0, nrd, Pp[0]);
+#pragma unroll 1
+    for (int it = 1; it <= 3; ++it) {
+        double fc[4];
+        q.advance(fm, it, fc, keep);
+        const double* __restrict__ xg = Xp + 4 * it * S;
+        double* __restrict__ pg = Pp + (4 * it - 3) * S;
+#pragma unroll
+        for (int e = 0; e < 4; ++e) {
+            w.push(xg[e * S]);
+            const double F = spt_face(w, fc[e]);
+            pg[e * S] = fma(F - Fprev, nrd, pg[e * S]);
+            Fprev = F;
+        }
+    }
+#pragma unroll
+    for (int e = 0; e < 3; ++e) {
+        w.push(hx[3 + e]);
+        const double F = spt_face(w, q.fn[e]);
+        Pp[(13 + e) * S] = fma(F - Fprev, nrd, Pp[(13 + e) * S]);
+        Fprev = F;
+    }
+}
+
+// x sweep: starts the partial sum; the pencil is a row of shared memory, read and written in pairs of zones
+__device__ __forceinline__ void spt_sweep_x(const double* __restrict__ Xp, double* __restrict__ Pp,
+                                            const double* __restrict__ fm, const double (&hx)[6], const double nrd,
+                                            const unsigned long long keep)
+{
+    PpmWindow w;
+    SptFm q;
+    q.start(fm, keep);
+    const double2 xa = *reinterpret_cast<const double2*>(Xp), xb = *reinterpret_cast<const double2*>(Xp + 2);
+    w.start(hx[0]); w.warm1(hx[1]); w.warm2(hx[2]);
+    w.warm3(xa.x);
+    w.push(xa.y);
+    w.push(xb.x);
+    const double F0 = spt_face(w, q.f0);
+    w.push(xb.y);
+    double Fprev = spt_face(w, q.f1);
+    double pend = fma(Fprev - F0, nrd, 0.0);                    // zone 0, stored with zone 1
+#pragma unroll 1
+    for (int it = 1; it <= 3; ++it) {
+        double fc[4];
+        q.advance(fm, it, fc, keep);
+        const double2 xc = *reinterpret_cast<const double2*>(Xp + 4 * it), xd = *reinterpret_cast<const double2*>(Xp + 4 * it + 2);
+        double* __restrict__ pg = Pp + 4 * it - 4;                 // zones 4it-4 .. 4it-1 complete in this group
+        double F, z, hold;
+        w.push(xc.x); F = spt_face(w, fc[0]); z = fma(F - Fprev, nrd, 0.0); Fprev = F;
+        *reinterpret_cast<double2*>(pg) = make_double2(pend, z);
+        w.push(xc.y); F = spt_face(w, fc[1]); hold = fma(F - Fprev, nrd, 0.0); Fprev = F;
+        w.push(xd.x); F = spt_face(w, fc[2]); z = fma(F - Fprev, nrd, 0.0); Fprev = F;
+        *reinterpret_cast<double2*>(pg + 2) = make_double2(hold, z);
+        w.push(xd.y); F = spt_face(w, fc[3]); pend = fma(F - Fprev, nrd, 0.0); Fprev = F;
+    }
+    {
+        double F, z, hold;
+        w.push(hx[3]); F = spt_face(w, q.fn[0]); z = fma(F - Fprev, nrd, 0.0); Fprev = F;
+        *reinterpret_cast<double2*>(Pp + 12) = make_double2(pend, z);
+        w.push(hx[4]); F = spt_face(w, q.fn[1]); hold = fma(F - Fprev, nrd, 0.0); Fprev = F;
+        w.push(hx[5]); F = spt_face(w, q.fn[2]); z = fma(F - Fprev, nrd, 0.0);
+        *reinterpret_cast<double2*>(Pp + 14) = make_double2(hold, z);
+    }
+}
+
+// write out component c_out of the tile from the partial-sum tile: A and, fused, U_next = U_m + ca A + sum c_r P_r.
+// Thread t takes the 16-byte piece t % 8 of rows t / 8 + 32 n (row = 16 k + j): every global access is a 16-byte vector.
+template <int NR>
+__device__ __forceinline__ void spt_write_out(const Geom& g, const TileCoord& tc, const double* __restrict__ Ps,
+                                              double* __restrict__ A, const UpdArgs& up, const int c_out)
+{
+    const int ng = CST_NG;
+    const int tid = threadIdx.x, cp = tid & 7, r0 = tid >> 3;
+    const unsigned long long strm = spt_policy_stream();
+    const long long zt = ((long long)(tc.k0 + ng) * g.ey + (tc.j0 + ng)) * g.ex + (tc.i0 + ng) + 2 * cp;
+    const long long arow = (long long)tc.b * g.box_a + (long long)c_out * g.comp_a +
+        ((long long)(tc.k0 + (r0 >> 4)) * g.ny + tc.j0 + (r0 & 15)) * g.nx + tc.i0 + 2 * cp;
+    const long long astep = 2LL * g.ny * g.nx;
+    const long long urow = (long long)tc.b * g.box_g + (long long)c_out * g.comp_g + zt +
+        (long long)(r0 >> 4) * g.plane_g + (long long)(r0 & 15) * g.ex;
+    const long long ustep = 2 * g.plane_g;
+    const double* pum = up.U_m + urow;
+    double* pun = up.U_next + urow;
+    double* pa = A + arow;
+    const double* pp[UPD_MAX_EXT];
+#pragma unroll
+    for (int r = 0; r < UPD_MAX_EXT; ++r) pp[r] = (r < NR) ? up.P[r] + arow : nullptr;
+    const double* ps = Ps + r0 * SPT_PITCH + 2 * cp;
+#pragma unroll
+    for (int n0 = 0; n0 < 8; n0 += 4) {
+        double2 um[4], pv[4][UPD_MAX_EXT];
+#pragma unroll
+        for (int e = 0; e < 4; ++e) {
+            if (NR >= 0) {
+                um[e] = spt_ldg2(pum);
+                pum += ustep;
+#pragma unroll
+                for (int r = 0; r < NR; ++r) { pv[e][r] = spt_ldg2(pp[r], strm); pp[r] += astep; }
+            }
+        }
+#pragma unroll
+        for (int e = 0; e < 4; ++e) {
+            const double2 av = *reinterpret_cast<const double2*>(ps + 32 * (n0 + e) * SPT_PITCH);
+            if (NR >= 0) {
+                double2 acc = make_double2(fma(up.ca, av.x, um[e].x), fma(up.ca, av.y, um[e].y));
+#pragma unroll
+                for (int r = 0; r < NR; ++r) {
+                    acc.x = fma(up.c[r], pv[e][r].x, acc.x); acc.y = fma(up.c[r], pv[e][r].y, acc.y);
+                }
+                spt_stg2(pun, acc, strm);
+                pun += ustep;
+            }
+            spt_stg2(pa, av, strm);
+            pa += astep;
+        }
+    }
+}
+
+// X = rho X / rho in place on the tile the TMA load has just delivered (waits for it on the mbarrier)
+__device__ __forceinline__ void spt_convert(const Geom& g, const TileCoord& tc, double* __restrict__ Xs,
+                                            const double* __restrict__ rinv_b, uint64_t* bar, const uint32_t parity,
+                                            const unsigned long long keep)
+{
+    const int ng = CST_NG;
+    const int tid = threadIdx.x, cp = tid & 7, r0 = tid >> 3;
+    const long long zrow = ((long long)(tc.k0 + ng + (r0 >> 4)) * g.ey + (tc.j0 + ng + (r0 & 15))) * g.ex + (tc.i0 + ng) + 2 * cp;
+    const double* pr = rinv_b + zrow;
+    double2 ri[8];
+#pragma unroll
+    for (int n = 0; n < 8; ++n) { ri[n] = spt_ldg2(pr, keep); pr += 2 * g.plane_g; }
+    mbar_wait(bar, parity);
+    double* x = Xs + r0 * SPT_PITCH + 2 * cp;
+#pragma unroll
+    for (int n = 0; n < 8; ++n) {
+        double2 v = *reinterpret_cast<const double2*>(x + 32 * n * SPT_PITCH);
+        v.x *= ri[n].x; v.y *= ri[n].y;
+        *reinterpret_cast<double2*>(x + 32 * n * SPT_PITCH) = v;
+    }
+}
+
+// the species [s_begin, s_end) of one full tile
+template <int NR>
+__device__ __forceinline__ void spt_tile(const Geom& g, const TileCoord& tc, const SptMaps& maps,
+                                         const double* __restrict__ Ub, const double* __restrict__ rinv_b,
+                                         const double* __restrict__ fm_tile, double* __restrict__ A, const UpdArgs& up,
+                                         double* __restrict__ sm, const int s_begin, const int s_end)
+{
+    const int ng = CST_NG;
+    double* XB = sm;                                  // [2][SPT_TILE]
+    double* PB = sm + 2 * SPT_TILE;                   // [SPT_TILE]
+    uint64_t* bar = reinterpret_cast<uint64_t*>(sm + 3 * SPT_TILE);
+    const int tid = threadIdx.x, a = tid & (TILE - 1), b = tid >> 4;
+    const int zc0 = (tc.b * g.nvar) * g.ez + tc.k0 + ng;      // z coordinate of component 0 in the U tensor map
+    const int za0 = (tc.b * g.nvar) * g.nz + tc.k0;           // ... in the A-like tensor maps
+    if (tid == 0) {
+        mbar_init(&bar[0], 1);
+        mbar_init(&bar[1], 1);
+        fence_mbar_init();
+        mbar_expect_tx(&bar[0], SPT_TILE_BYTES);
+        tma_load_3d(XB, &maps.u, tc.i0 + ng, tc.j0 + ng, zc0 + (5 + s_begin) * g.ez, &bar[0]);
+        // the tile's face mass fluxes and 1/rho star: one trip from HBM into L2 for all species passes
+        bulk_prefetch_l2(fm_tile, 3 * (TILE + 1) * NTHR * 8);
+        tma_prefetch_3d(&maps.r, tc.i0, tc.j0 + 1, tc.b * g.ez + tc.k0 + 1);
+    }
+    __syncthreads();
+    const double nrdx = -g.rdx, nrdy = -g.rdy, nrdz = -g.rdz;
+    const double* __restrict__ fm = fm_tile + tid;
+    int n = 0;
+#pragma unroll 1
+    for (int s = s_begin; s < s_end; ++s, ++n) {
+        const int c = 5 + s, cur = n & 1;
+        const bool last = (s + 1 >= s_end);
+        // 1/rho and Fm of this tile stay in L2 (evict_last) until the last species, which demotes them
+        const unsigned long long keep = last ? spt_policy_stream() : spt_policy_keep();
+        double* Xs = XB + cur * SPT_TILE;
+        const double* Us = Ub + (long long)c * g.comp_g;
+        if (n > 0) {
+            __syncthreads();                          // z sweep of the previous species done: P complete
+            spt_write_out<NR>(g, tc, PB, A, up, c - 1);
+        }
+        spt_convert(g, tc, Xs, rinv_b, &bar[cur], (n >> 1) & 1, keep);
+        SptHalo hr;
+        spt_halo_load(g, tc, 0, Us, rinv_b, hr, keep);
+        __syncthreads();                              // X complete; P and the other X buffer are free
+        if (tid == 0) {
+            if (!last) {
+                fence_proxy_async();
+                mbar_expect_tx(&bar[cur ^ 1], SPT_TILE_BYTES);
+                tma_load_3d(XB + (cur ^ 1) * SPT_TILE, &maps.u, tc.i0 + ng, tc.j0 + ng, zc0 + (c + 1) * g.ez, &bar[cur ^ 1]);
+            }
+            if (NR > 0) {                             // operands of this species' write-out: into L2 a pass ahead
+#pragma unroll
+                for (int r = 0; r < NR; ++r) tma_prefetch_3d(&maps.p[r], tc.i0, tc.j0, za0 + c * g.nz);
+            }
+        }
+        double hx[6];
+        // ---- x sweep
+#pragma unroll
+        for (int m = 0; m < 6; ++m) hx[m] = hr.u[m] * hr.r[m];
+        spt_halo_load(g, tc, 1, Us, rinv_b, hr, keep);          // operands of the y sweep: in flight during the x sweep
+        spt_sweep_x(Xs + spt_sbase<0>(a, b), PB + spt_sbase<0>(a, b), fm, hx, nrdx, keep);
+        __syncthreads();
+        // ---- y sweep
+#pragma unroll
+        for (int m = 0; m < 6; ++m) hx[m] = hr.u[m] * hr.r[m];
+        spt_halo_load(g, tc, 2, Us, rinv_b, hr, keep);
+        spt_sweep_yz<1>(Xs + spt_sbase<1>(a, b), PB + spt_sbase<1>(a, b), fm + (TILE + 1) * NTHR, hx, nrdy, keep);
+        __syncthreads();
+        // ---- z sweep
+#pragma unroll
+        for (int m = 0; m < 6; ++m) hx[m] = hr.u[m] * hr.r[m];
+        spt_sweep_yz<2>(Xs + spt_sbase<2>(a, b), PB + spt_sbase<2>(a, b), fm + 2 * (TILE + 1) * NTHR, hx, nrdz, keep);
+    }
+    __syncthreads();
+    spt_write_out<NR>(g, tc, PB, A, up, 5 + s_end - 1);
+}

@@ -1,18 +1,25 @@
 """Parity at BASELINE.json's FULL sizes, in the launch configuration bench.py times (the fused
-cst_advance_A_update with two distinct A_old arrays), on SAMPLED outputs: sub-boxes of the domain
-are cut out of the GPU's ghost-filled state (with their 4-deep halo), the oracle evaluates A and the
-node update on each sub-box as a stand-alone box, and the GPU's A / U_next are compared there.
-Gate as everywhere: per component max|gpu - orc| / max|orc| <= 1e-12 (over the sampled zones)."""
+cst_advance_A_update with two distinct A_old arrays), over EVERY zone of configs[1..3] and over EVERY box of
+configs[4] (SURVEY 8(d) "Parity harness per config").
+
+The oracle cannot hold a whole 512^3 x 18 state, so single-box configs are streamed in k-slabs: `sk` interior
+planes plus the 4-deep halo are cut out of the GPU's ghost-FILLED state and handed to the oracle as a stand-alone
+box (A needs only the +-3 star, so the slab's ghosts are exactly the halo); box batches go box by box.  A and
+U_next are pre-filled with NaN, so a tile that no CTA writes (or the wrong CTA writes) shows up at once.
+Gate as everywhere: per component max|gpu - orc| / max|orc| <= 1e-12 (maxima over the whole config).
+The multi-step runs of the configs' own definitions (50 / 20 / 10 SDC steps) follow, in lock-step with the oracle.
+"""
 import numpy as np
 import pytest
 import torch
 
 from oracle import orc
-from paper_1910_12578_b200 import Context, workloads as wl
+from paper_1910_12578_b200 import Context, sdc_step_2nd, workloads as wl
 
 pytestmark = pytest.mark.gpu
 DEV = "cuda:0"
 TOL = 1e-12
+NG = 4
 
 
 def need_gb(gb):
@@ -32,65 +39,241 @@ def device_state(cfg):
     return U
 
 
-def check_samples(cfg, samples, sub=16):
-    """samples: list of (box, k0, j0, i0) interior origins of sub x sub x sub sub-boxes."""
+class ErrAcc:
+    """running per-component max |gpu - orc| and max |orc| (the Q21 norm over everything that was fed)"""
+
+    def __init__(self, N):
+        self.num, self.den = np.zeros(N), np.zeros(N)
+
+    def add(self, gpu, ref):          # arrays [c][...]
+        ax = tuple(range(1, ref.ndim))
+        self.num = np.maximum(self.num, np.abs(gpu - ref).max(axis=ax))
+        self.den = np.maximum(self.den, np.abs(ref).max(axis=ax))
+
+    def err(self):
+        return np.where(self.den > 0, self.num / np.where(self.den > 0, self.den, 1.0), self.num)
+
+
+def run_fused(cfg):
+    """fill + cfl + fused advance in bench.py's launch configuration; outputs pre-filled with NaN."""
     ctx = Context(cfg)
     U = device_state(cfg)
     ctx.fill_ghosts(U)
     dt = ctx.cfl_dt(U, 0.5)
     ash = wl.a_shape(cfg)
-    A, A0, A1 = (torch.empty(ash, dtype=torch.float64, device=DEV) for _ in range(3))
+    A0 = torch.empty(ash, dtype=torch.float64, device=DEV)
     ctx.advance_A(U, A0)                       # plausible A_old values, as in bench.py
-    A1.copy_(A0).mul_(0.9)
-    Un = torch.zeros_like(U)
+    A1 = A0 * 0.9
+    A = torch.full(ash, float("nan"), dtype=torch.float64, device=DEV)
+    Un = torch.full(wl.u_shape(cfg), float("nan"), dtype=torch.float64, device=DEV)
     w = [0.5 * dt, 0.5 * dt]
     ctx.advance_A_update(U, A, Un, dt, A0, [A0, A1], w)
     torch.cuda.synchronize()
-    N, ng = wl.nvar(cfg), 4
-    sc = dict(cfg, nx=sub, ny=sub, nz=sub, nbx=1, nby=1, nbz=1)
-    numA, denA, numU, denU = (np.zeros(N) for _ in range(4))
-    for (b, k0, j0, i0) in samples:
-        Us = U[b, :, k0:k0 + sub + 2 * ng, j0:j0 + sub + 2 * ng, i0:i0 + sub + 2 * ng].cpu().numpy()[None].copy()
-        sl = (b, slice(None), slice(k0, k0 + sub), slice(j0, j0 + sub), slice(i0, i0 + sub))
+    # every output zone written, nothing else touched
+    assert torch.isfinite(A).all(), "unwritten zones in A"
+    nint = int(np.prod(ash))
+    assert int(torch.isfinite(Un).sum()) == nint, "U_next: interior not fully written or ghosts touched"
+    assert torch.isfinite(Un[:, :, NG:-NG, NG:-NG, NG:-NG]).all()
+    return ctx, U, A, A0, A1, Un, dt, w
+
+
+def check_periodic_sums(cfg, A):
+    """whole-array invariant at zero oracle cost: sum_zones A_c = 0 on periodic domains without gravity"""
+    if any(b != 0 for b in cfg["bc_lo"]) or any(g != 0.0 for g in cfg["grav"]):
+        return
+    s = A.sum(dim=(0, 2, 3, 4)).cpu().numpy()
+    sa = A.abs().sum(dim=(0, 2, 3, 4)).cpu().numpy()
+    assert np.all(np.abs(s) <= 1e-11 * sa), s / sa
+
+
+def check_single_box_all_slabs(cfg, sk):
+    ctx, U, A, A0, A1, Un, dt, w = run_fused(cfg)
+    check_periodic_sums(cfg, A)
+    N, nz = wl.nvar(cfg), cfg["nz"]
+    eA, eU = ErrAcc(N), ErrAcc(N)
+    for k0 in range(0, nz, sk):
+        n = min(sk, nz - k0)
+        sc = dict(cfg, nz=n)
+        Us = U[:, :, k0:k0 + n + 2 * NG].cpu().numpy()
         Ao = orc.advance_A(sc, Us)
-        Ag, A0s, A1s = (x[sl].cpu().numpy()[None] for x in (A, A0, A1))
-        # the GPU's A_old0 was computed by the GPU; the update is checked from bit-identical inputs
+        Ag, A0s, A1s = (x[:, :, k0:k0 + n].cpu().numpy() for x in (A, A0, A1))
+        eA.add(Ag[0], Ao[0])
         Uno = Us.copy()
-        orc.sdc_update(sc, Uno, Us, dt, Ao, A0s, [A0s, A1s], w)
-        Ung = Un[b, :, k0 + ng:k0 + ng + sub, j0 + ng:j0 + ng + sub, i0 + ng:i0 + ng + sub].cpu().numpy()
-        Uni = Uno[0, :, ng:ng + sub, ng:ng + sub, ng:ng + sub]
-        ax = (1, 2, 3)
-        numA = np.maximum(numA, np.abs(Ag[0] - Ao[0]).max(axis=ax)); denA = np.maximum(denA, np.abs(Ao[0]).max(axis=ax))
-        numU = np.maximum(numU, np.abs(Ung - Uni).max(axis=ax)); denU = np.maximum(denU, np.abs(Uni).max(axis=ax))
-    eA, eU = (numA / denA).max(), (numU / denU).max()
-    print(cfg["name"], "sampled sub-boxes", len(samples), "A err", eA, "U_next err", eU)
-    assert eA <= TOL and eU <= TOL, (numA / denA, numU / denU)
+        orc.sdc_update(sc, Uno, Us, dt, Ao, A0s, [A0s, A1s], w)     # from the ORACLE's A: bit-identical inputs
+        Ung = Un[0, :, k0 + NG:k0 + NG + n, NG:-NG, NG:-NG].cpu().numpy()
+        eU.add(Ung, Uno[0, :, NG:NG + n, NG:-NG, NG:-NG])
+    print(cfg["name"], "all", nz // sk, "slabs: A err", eA.err().max(), "U_next err", eU.err().max())
+    assert eA.err().max() <= TOL and eU.err().max() <= TOL, (eA.err(), eU.err())
     ctx.destroy()
 
 
-def test_configs3_512_sampled():
+def test_configs1_128_every_zone():
+    check_single_box_all_slabs(wl.make_config(1), sk=32)
+
+
+def test_configs2_256_every_zone():
+    need_gb(8)
+    check_single_box_all_slabs(wl.make_config(2), sk=32)
+
+
+def test_configs3_512_every_zone():
     need_gb(110)
-    cfg = wl.make_config(3)
-    s = [(0, 0, 0, 0), (0, 496, 496, 496), (0, 248, 8, 496), (0, 100, 300, 16), (0, 8, 250, 250), (0, 333, 77, 129)]
-    check_samples(cfg, s)
+    check_single_box_all_slabs(wl.make_config(3), sk=16)
 
 
-def test_configs4_boxes_sampled():
+def test_configs4_every_box():
+    """all 512 boxes of the batch, each evaluated by the oracle as a stand-alone box from the GPU's filled state
+    (covers the reflecting z walls of every column, the periodic x / y wraps and every interior box face)"""
     need_gb(122)
     cfg = wl.make_config(4)
-    # boxes at the reflecting z walls, at periodic x/y wraps and in the interior; sub-boxes touching box faces
-    s = [(0, 0, 0, 0), (511, 48, 48, 48), (16 * 8 * 3 + 5, 48, 0, 20), (130, 20, 48, 0), (257, 24, 24, 24), (15, 0, 30, 48)]
-    check_samples(cfg, s)
+    ctx, U, A, A0, A1, Un, dt, w = run_fused(cfg)
+    N = wl.nvar(cfg)
+    bc = dict(cfg, nbx=1, nby=1, nbz=1)
+    eA, eU = ErrAcc(N), ErrAcc(N)
+    for b in range(U.shape[0]):
+        Us = U[b:b + 1].cpu().numpy()
+        Ao = orc.advance_A(bc, Us)
+        Ag, A0s, A1s = (x[b:b + 1].cpu().numpy() for x in (A, A0, A1))
+        eA.add(Ag[0], Ao[0])
+        Uno = Us.copy()
+        orc.sdc_update(bc, Uno, Us, dt, Ao, A0s, [A0s, A1s], w)
+        eU.add(Un[b, :, NG:-NG, NG:-NG, NG:-NG].cpu().numpy(), Uno[0, :, NG:-NG, NG:-NG, NG:-NG])
+    print(cfg["name"], "all boxes: A err", eA.err().max(), "U_next err", eU.err().max())
+    assert eA.err().max() <= TOL and eU.err().max() <= TOL, (eA.err(), eU.err())
+    ctx.destroy()
 
 
-def test_configs2_256_sampled():
-    need_gb(8)
-    cfg = wl.make_config(2)
-    s = [(0, 120, 120, 120), (0, 0, 0, 0), (0, 240, 240, 240), (0, 128, 100, 150), (0, 112, 128, 128)]
-    check_samples(cfg, s)
+# ------------------------------------------------------------------ multi-step, the configs' own definitions ----
+def comp_err(gpu, ref):
+    axes = (0, 2, 3, 4)
+    num, den = np.abs(gpu - ref).max(axis=axes), np.abs(ref).max(axis=axes)
+    return np.where(den > 0, num / np.where(den > 0, den, 1.0), num)
 
 
-def test_configs1_128_sampled():
+def interior(U):
+    return U[:, :, NG:-NG, NG:-NG, NG:-NG]
+
+
+def lockstep(cfg, steps, ctx=None):
+    """Every step both sides start from the ORACLE's current state; each step of the GPU (ghost fill, two A
+    evaluations, two node updates) must reproduce the oracle's new state to 1e-12.  Returns
+    the oracle's final state and the elapsed time."""
+    ctx = ctx or Context(cfg)
+    Uo = orc.fill_ghosts(cfg, wl.initial_state(cfg))
+    ash = wl.a_shape(cfg)
+    Ul = torch.empty(wl.u_shape(cfg), dtype=torch.float64, device=DEV)
+    U1 = torch.empty_like(Ul)
+    A0, A1 = (torch.empty(ash, dtype=torch.float64, device=DEV) for _ in range(2))
+    t, worst = 0.0, 0.0
+    for step in range(steps):
+        dt = orc.cfl_dt(cfg, Uo, cfg["cfl"])
+        Ul.copy_(torch.from_numpy(Uo))
+        dtg = ctx.cfl_dt(Ul, cfg["cfl"])
+        assert abs(dtg - dt) <= 1e-14 * dt
+        sdc_step_2nd(ctx, Ul, U1, A0, A1, dt)
+        Uo = orc.fill_ghosts(cfg, orc.sdc_step_2nd(cfg, Uo, dt))
+        e = comp_err(interior(Ul.cpu().numpy()), interior(Uo))
+        worst = max(worst, e.max())
+        assert e.max() <= TOL, (cfg["name"], step, e)
+        t += dt
+    print(cfg["name"], steps, "lock-steps: worst per-step error", worst)
+    return Uo, t
+
+
+def free_run(cfg, steps, ctx=None):
+    ctx = ctx or Context(cfg)
+    Ug = device_state(cfg)
+    U1 = torch.empty_like(Ug)
+    A0, A1 = (torch.empty(wl.a_shape(cfg), dtype=torch.float64, device=DEV) for _ in range(2))
+    t = 0.0
+    for _ in range(steps):
+        dt = ctx.cfl_dt(Ug, cfg["cfl"])
+        sdc_step_2nd(ctx, Ug, U1, A0, A1, dt)
+        t += dt
+    return Ug, t
+
+
+def test_configs1_128_50_steps_lockstep_and_exact_solution():
+    """configs[1] as defined: 128^3 oblique Sod, outflow, 50 SDC steps.  Lock-step parity of every step; the GPU's
+    own free-running density is then compared with the exact Riemann solution along the normal in the central cube
+    (within 2 % of the oracle's L1 error)."""
     cfg = wl.make_config(1)
-    s = [(0, 56, 56, 56), (0, 0, 0, 0), (0, 112, 112, 112), (0, 40, 60, 80)]
-    check_samples(cfg, s)
+    ctx = Context(cfg)
+    Uo, t = lockstep(cfg, cfg["steps"], ctx)
+    Ug, tg = free_run(cfg, cfg["steps"], ctx)
+    assert abs(tg - t) <= 1e-9 * t
+    n = cfg["nx"]
+    G, Go = interior(Ug.cpu().numpy())[0, 0], interior(Uo)[0, 0]
+    drift = np.abs(G - Go).max() / np.abs(Go).max()
+    x = (np.arange(n) + 0.5) / n
+    Z, Y, X = np.meshgrid(x, x, x, indexing="ij")
+    xi = ((X + Y + Z - 1.5) / np.sqrt(3.0)) / t
+    re, _, _ = orc.exact_riemann_sample(1.4, 1.0, 0.0, 1.0, 0.125, 0.0, 0.1, xi.ravel())
+    re = re.reshape(n, n, n)
+    cen = (np.abs(X - 0.5) < 0.25) & (np.abs(Y - 0.5) < 0.25) & (np.abs(Z - 0.5) < 0.25)
+    l1_g, l1_o = np.abs(G - re)[cen].mean(), np.abs(Go - re)[cen].mean()
+    print("configs[1] free-running drift", drift, "central L1 gpu/oracle", l1_g, l1_o)
+    assert drift < 1e-9                                  # reported; an end-state 1e-12 gate is unattainable (Q21)
+    assert abs(l1_g - l1_o) <= 0.02 * l1_o and l1_g < 0.02
+
+
+def test_configs2_256_20_steps_lockstep_conservation_and_order():
+    """configs[2] as defined: 256^3 Gaussian pulse, periodic, 20 steps in lock-step; conservation of the GPU's
+    free run; second-order convergence (P15) from the GPU's OWN 64^3 / 128^3 results at a fixed end time."""
+    need_gb(12)
+    cfg = wl.make_config(2)
+    ctx = Context(cfg)
+    lockstep(cfg, cfg["steps"], ctx)
+    Ug0 = device_state(cfg)
+    tot0 = interior(Ug0).sum(dim=(0, 2, 3, 4)).cpu().numpy()
+    Ug, _ = free_run(cfg, cfg["steps"], ctx)
+    Ui = interior(Ug)
+    tot1 = Ui.sum(dim=(0, 2, 3, 4)).cpu().numpy()
+    assert np.all(np.abs(tot1 - tot0) <= 1e-13 * Ui.abs().sum(dim=(0, 2, 3, 4)).cpu().numpy())
+    ctx.destroy()
+    del Ug, Ug0, Ui
+
+    def l1_at(n, t_end=0.05):
+        c = wl.make_config(2, n=n)
+        cx = Context(c)
+        U = device_state(c)
+        U1 = torch.empty_like(U)
+        A0, A1 = (torch.empty(wl.a_shape(c), dtype=torch.float64, device=DEV) for _ in range(2))
+        t = 0.0
+        while t < t_end * (1 - 1e-12):
+            dt = min(cx.cfl_dt(U, 0.5), t_end - t)
+            sdc_step_2nd(cx, U, U1, A0, A1, dt)
+            t += dt
+        x = (np.arange(n) + 0.5) / n
+        Z, Y, X = np.meshgrid(x, x, x, indexing="ij")
+        per = lambda a: (a - t_end - 0.5 + 0.5) % 1.0 - 0.5            # periodic distance to the moved centre
+        r2 = per(X) ** 2 + per(Y) ** 2 + per(Z) ** 2
+        exact = 1.0 + 0.5 * np.exp(-r2 / 0.01)
+        return np.abs(interior(U.cpu().numpy())[0, 0] - exact).mean()
+    e32, e64, e128 = l1_at(32), l1_at(64), l1_at(128)
+    print("configs[2] L1 at 32/64/128 on the GPU:", e32, e64, e128, "ratios", e32 / e64, e64 / e128)
+    assert e64 / e128 >= 3.5
+
+
+def test_configs4_10_steps_lockstep_column_and_free_run_batch():
+    """configs[4] as defined, 10 SDC steps with gravity and reflecting z walls evolving: lock-step on a 2 x 2 x 4
+    column of the 64^3 boxes (full height, 13 species); then the full 512-box batch runs free on the GPU and the
+    interior vertical Mach number must stay below 1e-3 (the walls themselves reach ~1e-2)."""
+    cfg = wl.make_config(4, nb=(2, 2, 4))
+    lockstep(cfg, cfg["steps"])
+    need_gb(125)
+    full = wl.make_config(4)
+    Ug, _ = free_run(full, full["steps"])
+    worst = 0.0
+    for bk in range(full["nbz"]):
+        for b in range(bk * full["nbx"] * full["nby"], (bk + 1) * full["nbx"] * full["nby"], 7):
+            Ub = Ug[b, :5, NG:-NG, NG:-NG, NG:-NG]
+            k_lo = 16 if bk == 0 else 0                       # keep 16 zones away from either wall
+            k_hi = full["nz"] - 16 if bk == full["nbz"] - 1 else full["nz"]
+            Ub = Ub[:, k_lo:k_hi]
+            rho, w = Ub[0], Ub[3] / Ub[0]
+            p = (full["gamma"] - 1) * (Ub[4] - 0.5 * (Ub[1] ** 2 + Ub[2] ** 2 + Ub[3] ** 2) / rho)
+            assert bool((p > 0).all()) and bool((rho > 0).all())
+            worst = max(worst, float((w.abs() / torch.sqrt(full["gamma"] * p / rho)).max()))
+    print("configs[4] free run, 10 steps: interior max |w|/c =", worst)
+    assert worst < 1e-3
