@@ -166,7 +166,7 @@ static int launch_species_nr(cst_ctx* ctx, const double* U, double* A, const Upd
     SptMaps maps;
     if (tma) {
         const unsigned long long nbv = (unsigned long long)g.nbox * g.nvar;
-        tma = tma_encode_3d_f64(&maps.u, U, g.ex, g.ey, nbv * g.ez, SPT_PITCH, TILE, TILE) &&
+        tma = tma_encode_3d_f64(&maps.u, U, g.ex, g.ey, nbv * g.ez, SPT_XW, TILE, TILE) &&
               tma_encode_3d_f64(&maps.r, rinv, g.ex, g.ey, (unsigned long long)g.nbox * g.ez, 24, 22, 22);
         for (int r = 0; r < UPD_MAX_EXT; ++r)
             maps.p[r] = maps.u;                               // unused slots: any valid map

@@ -1,30 +1,39 @@
 // species_tma.cuh -- fast path of the species kernel for boxes made of full 16^3 tiles (k_advect_species_tma).
 //
 // One CTA (256 threads) works on one 16^3 tile and a contiguous share of the species; two CTAs share an SM.  Per species:
-//   * rho X of the tile core arrives by ONE tensor-map (TMA) tile load -- issued a whole species pass earlier, double
-//     buffered, completing on an mbarrier -- so no compute warp ever waits for HBM on it;
+//   * rho X of the tile core PLUS its x halos arrives by ONE tensor-map (TMA) tile load (box 24 x 16 x 16: zones -4 .. 19
+//     of every x pencil -- a box must start on a 16-byte boundary, measured: an odd fp64 start coordinate faults),
+//     completing on an mbarrier; the box was pulled into L2 by a tensor prefetch a whole species pass earlier and the
+//     load itself is issued as soon as the previous species' z sweep has released the buffer, so it overlaps the
+//     write-out of that species;
 //   * the face mass fluxes Fm, 1/rho and the fused update's operands (A_old arrays) are pulled into L2 by bulk / tensor
 //     prefetches one pass ahead of the loads that use them;
-//   * X = rho X / rho is formed in place, then three sweeps (x, y, z), one pencil per thread with the PPM window in
-//     registers (sweep.cuh), accumulate -div F into the partial-sum tile; the next pass writes A (and U_next) out.
-// Shared-memory tiles are dense rows of 18 doubles (144 bytes: the TMA box is 18 zones wide): every access of every
-// sweep is "pencil base + immediate", rows stay 16-byte aligned, the x sweep reads and writes PAIRS of zones (16-byte
-// accesses: eight threads of a quarter warp hit eight different 16-byte bank groups because 9 j mod 8 is a permutation),
-// and the y / z sweeps touch 16 consecutive doubles per half warp -- no bank conflicts, no swizzle arithmetic.
+//   * X = rho X / rho is formed in place (halo columns included), then three sweeps (x, y, z), one pencil per thread
+//     with the PPM window in registers (sweep.cuh), accumulate -div F into the partial-sum tile; the next pass writes
+//     A (and U_next) out.
+// Shared memory: the X tile has dense rows of 24 doubles (x = -4 .. 19), the partial-sum tile rows of 18 doubles (84 KB per
+// CTA, 168 KB per SM: the L1 that is left still carries the remaining per-thread global loads -- at 216 KB the same
+// kernel ran 1.4x slower).  Every access of every sweep is "pencil base + immediate"; rows stay 16-byte aligned; the x
+// sweep reads and writes PAIRS of zones (16-byte accesses; the partial-sum rows are conflict free because 9 j mod 8 is a
+// permutation, the twelve X reads per pencil pay a 4-way conflict: 3 % of the sweep); the y / z sweeps touch 16 consecutive
+// doubles per half warp -- no swizzle arithmetic, and the x halos never travel through registers.
 // Same arithmetic, zone for zone, as species_sweep (advect_species.cu) and as the oracle's S1-S5.
 #pragma once
 #include "sweep.cuh"
 #include "tile.cuh"
 #include "tma.cuh"
 
-#define SPT_PITCH 18
+#define SPT_XW 24                             // X tile row: zones -4 .. 19 of the x pencil
+#define SPT_XPLANE (TILE * SPT_XW)            // 384 doubles
+#define SPT_XTILE (TILE * SPT_XPLANE)         // 6144 doubles
+#define SPT_XTILE_BYTES (SPT_XTILE * 8)       // 49152 = the TMA box 24 x 16 x 16
+#define SPT_PITCH 18                          // partial-sum tile row (zones 0 .. 15 + 2 pad)
 #define SPT_PLANE (TILE * SPT_PITCH)          // 288 doubles
 #define SPT_TILE (TILE * SPT_PLANE)           // 4608 doubles
-#define SPT_TILE_BYTES (SPT_TILE * 8)         // 36864 = the TMA box 18 x 16 x 16
-#define SPT_SMEM (3 * SPT_TILE_BYTES + 128)   // X[2], P, two mbarriers
+#define SPT_SMEM (SPT_XTILE_BYTES + SPT_TILE * 8 + 128)   // X, P, one mbarrier
 
 struct SptMaps {             // tensor maps of one call (host-encoded, passed as a __grid_constant__ kernel parameter)
-    CUtensorMap u;           // U as [nbox*nvar*ez][ey][ex], box 18 x 16 x 16: the tile-core load
+    CUtensorMap u;           // U as [nbox*nvar*ez][ey][ex], box 24 x 16 x 16: tile core + x halos (load and L2 prefetch)
     CUtensorMap r;           // 1/rho workspace as [nbox*ez][ey][ex], box 24 x 22 x 22: L2 prefetch of the tile's star
     CUtensorMap p[UPD_MAX_EXT];   // external arrays of the fused update as [nbox*nvar*nz][ny][nx], box 16^3: L2 prefetch
 };
@@ -64,27 +73,35 @@ __device__ __forceinline__ void spt_stg2(double* a, double2 v, unsigned long lon
     asm volatile("st.global.L2::cache_hint.v2.f64 [%0], {%1,%2}, %3;" :: "l"(a), "d"(v.x), "d"(v.y), "l"(pol) : "memory");
 }
 
-// pencil of this thread in direction D: (a, b) = (tid % 16, tid / 16) = (j, k) | (i, k) | (i, j)
-template <int D> struct SptDir { static constexpr int SST = (D == 0) ? 1 : (D == 1) ? SPT_PITCH : SPT_PLANE; };
-
+// Pencil of this thread in direction D: (a, b) = (tid % 16, tid / 16) = (j, k) | (i, k) | (i, j).
+// X tile: zone (k, j, x) at k * SPT_XPLANE + j * SPT_XW + (x + 4), x = -4 .. 19; P tile: zone (k, j, i) at
+// k * SPT_PLANE + j * SPT_PITCH + i.
+template <int D> struct SptDir {
+    static constexpr int XS = (D == 0) ? 1 : (D == 1) ? SPT_XW : SPT_XPLANE;        // X stride along the pencil
+    static constexpr int PS = (D == 0) ? 1 : (D == 1) ? SPT_PITCH : SPT_PLANE;      // P stride along the pencil
+};
 template <int D>
-__device__ __forceinline__ int spt_sbase(const int a, const int b)
-{   // shared-memory index (doubles) of pencil position 0
+__device__ __forceinline__ int spt_xbase(const int a, const int b)
+{   // X index of pencil position 0 (D = 0: of position -4, the start of the row)
+    return (D == 0) ? (b * TILE + a) * SPT_XW : (D == 1) ? b * SPT_XPLANE + a + 4 : b * SPT_XW + a + 4;
+}
+template <int D>
+__device__ __forceinline__ int spt_pbase(const int a, const int b)
+{
     return (D == 0) ? (b * TILE + a) * SPT_PITCH : (D == 1) ? b * SPT_PLANE + a : b * SPT_PITCH + a;
 }
 
 struct SptHalo { double u[6], r[6]; };      // raw rho X and 1/rho at pencil positions -3..-1 (0..2) and 16..18 (3..5)
 
-// halo operands of this thread's pencil in direction d (run time), straight from global memory: requested one sweep
-// before they are used
+// halo operands of this thread's y (d = 1) or z (d = 2) pencil, straight from global memory (16 consecutive doubles
+// per half warp): requested one sweep before they are used
 __device__ __forceinline__ void spt_halo_load(const Geom& g, const TileCoord& tc, const int d, const double* __restrict__ Us,
                                               const double* __restrict__ rinv_b, SptHalo& h, const unsigned long long keep)
 {
     const int ng = CST_NG, a = threadIdx.x & (TILE - 1), b = threadIdx.x >> 4;
     const long long zt = ((long long)(tc.k0 + ng) * g.ey + (tc.j0 + ng)) * g.ex + (tc.i0 + ng);
     long long z0, stride;
-    if (d == 0) { z0 = zt + b * g.plane_g + (long long)a * g.ex; stride = 1; }
-    else if (d == 1) { z0 = zt + b * g.plane_g + a; stride = g.ex; }
+    if (d == 1) { z0 = zt + b * g.plane_g + a; stride = g.ex; }
     else { z0 = zt + (long long)b * g.ex + a; stride = g.plane_g; }
 #pragma unroll
     for (int n = 0; n < 6; ++n) {
@@ -99,93 +116,90 @@ __device__ __forceinline__ double spt_face(const PpmWindow& w, const double fmc)
     return fmc * (sign_bit(fmc) ? w.qm : w.qpL);
 }
 
-// face mass fluxes of one pencil: thread-private slots fm[f * NTHR], f = 0..16, requested two groups of four ahead
-struct SptFm {
-    double f0, f1, fn[4], fnn[4];
-    __device__ __forceinline__ void start(const double* __restrict__ fm, const unsigned long long keep)
-    {
-        f0 = spt_ldg(fm, keep); f1 = spt_ldg(fm + NTHR, keep);
+// y or z sweep: X and P of pencil position p at Xp[p * XS], Pp[p * PS] (compile-time strides).  Face mass fluxes of
+// the pencil: thread-private slots fm[f * NTHR], f = 0..16, requested two groups of four ahead of their use.
+template <int D>
+__device__ __forceinline__ void spt_sweep_yz(const double* __restrict__ Xp, double* __restrict__ Pp,
+                                             const double* __restrict__ fm, const double (&hx)[6], const double nrd,
+                                             const unsigned long long keep)
+{
+    constexpr int XS = SptDir<D>::XS, PS = SptDir<D>::PS;
+    PpmWindow w;
+    double fn[4], fnn[4];
+    const double f0 = spt_ldg(fm, keep), f1 = spt_ldg(fm + NTHR, keep);
 #pragma unroll
-        for (int e = 0; e < 4; ++e) fn[e] = spt_ldg(fm + (2 + e) * NTHR, keep);
+    for (int e = 0; e < 4; ++e) fn[e] = spt_ldg(fm + (2 + e) * NTHR, keep);
 #pragma unroll
-        for (int e = 0; e < 4; ++e) fnn[e] = spt_ldg(fm + (6 + e) * NTHR, keep);
-    }
-    // at the top of loop iteration it (1..3): fc <- faces 4it-2 .. 4it+1, and the request for faces 4it+6 ..
-    __device__ __forceinline__ void advance(const double* __restrict__ fm, const int it, double (&fc)[4], const unsigned long long keep)
-    {
+    for (int e = 0; e < 4; ++e) fnn[e] = spt_ldg(fm + (6 + e) * NTHR, keep);
+    w.start(hx[0]); w.warm1(hx[1]); w.warm2(hx[2]);
+    w.warm3(Xp[0]);
+    w.push(Xp[XS]);
+    w.push(Xp[2 * XS]);
+    const double F0 = spt_face(w, f0);
+    w.push(Xp[3 * XS]);
+    double Fprev = spt_face(w, f1);
+    Pp[0] = fma(Fprev - F0, nrd, Pp[0]);
+#pragma unroll 1
+    for (int it = 1; it <= 3; ++it) {                 // positions 4it .. 4it+3: faces 4it-2 .., zones 4it-3 ..
+        double fc[4];
 #pragma unroll
         for (int e = 0; e < 4; ++e) {
             fc[e] = fn[e];
             fn[e] = fnn[e];
             if (it < 2 || (it == 2 && e < 3)) fnn[e] = spt_ldg(fm + (4 * it + 6 + e) * NTHR, keep);
         }
-    }
-};
-
-// y or z sweep: X and P of pencil position p at Xp[p * SST], Pp[p * SST] (compile-time strides)
-template <int D>
-__device__ __forceinline__ void spt_sweep_yz(const double* __restrict__ Xp, double* __restrict__ Pp,
-                                             const double* __restrict__ fm, const double (&hx)[6], const double nrd,
-                                             const unsigned long long keep)
-{
-    constexpr int S = SptDir<D>::SST;
-    PpmWindow w;
-    SptFm q;
-    q.start(fm, keep);
-    w.start(hx[0]); w.warm1(hx[1]); w.warm2(hx[2]);
-    w.warm3(Xp[0]);
-    w.push(Xp[S]);
-    w.push(Xp[2 * S]);
-    const double F0 = spt_face(w, q.f0);
-    w.push(Xp[3 * S]);
-    double Fprev = spt_face(w, q.f1);
-    Pp[0] = fma(Fprev - F0, nrd, Pp[0]);
-#pragma unroll 1
-    for (int it = 1; it <= 3; ++it) {
-        double fc[4];
-        q.advance(fm, it, fc, keep);
-        const double* __restrict__ xg = Xp + 4 * it * S;
-        double* __restrict__ pg = Pp + (4 * it - 3) * S;
+        const double* __restrict__ xg = Xp + 4 * it * XS;
+        double* __restrict__ pg = Pp + (4 * it - 3) * PS;
 #pragma unroll
         for (int e = 0; e < 4; ++e) {
-            w.push(xg[e * S]);
+            w.push(xg[e * XS]);
             const double F = spt_face(w, fc[e]);
-            pg[e * S] = fma(F - Fprev, nrd, pg[e * S]);
+            pg[e * PS] = fma(F - Fprev, nrd, pg[e * PS]);
             Fprev = F;
         }
     }
 #pragma unroll
     for (int e = 0; e < 3; ++e) {
         w.push(hx[3 + e]);
-        const double F = spt_face(w, q.fn[e]);
-        Pp[(13 + e) * S] = fma(F - Fprev, nrd, Pp[(13 + e) * S]);
+        const double F = spt_face(w, fn[e]);
+        Pp[(13 + e) * PS] = fma(F - Fprev, nrd, Pp[(13 + e) * PS]);
         Fprev = F;
     }
 }
 
-// x sweep: starts the partial sum; the pencil is a row of shared memory, read and written in pairs of zones
-__device__ __forceinline__ void spt_sweep_x(const double* __restrict__ Xp, double* __restrict__ Pp,
-                                            const double* __restrict__ fm, const double (&hx)[6], const double nrd,
-                                            const unsigned long long keep)
+// x sweep: starts the partial sum.  The pencil is one row of the X tile, halos included: Xr[o] = X at position o - 4,
+// read as twelve pairs (positions (2m-4, 2m-3) in pair m); the row of P is written as eight pairs.
+__device__ __forceinline__ void spt_sweep_x(const double* __restrict__ Xr, double* __restrict__ Pp,
+                                            const double* __restrict__ fm, const double nrd, const unsigned long long keep)
 {
     PpmWindow w;
-    SptFm q;
-    q.start(fm, keep);
-    const double2 xa = *reinterpret_cast<const double2*>(Xp), xb = *reinterpret_cast<const double2*>(Xp + 2);
-    w.start(hx[0]); w.warm1(hx[1]); w.warm2(hx[2]);
+    double fn[4], fnn[4];
+    const double f0 = spt_ldg(fm, keep), f1 = spt_ldg(fm + NTHR, keep);
+#pragma unroll
+    for (int e = 0; e < 4; ++e) fn[e] = spt_ldg(fm + (2 + e) * NTHR, keep);
+#pragma unroll
+    for (int e = 0; e < 4; ++e) fnn[e] = spt_ldg(fm + (6 + e) * NTHR, keep);
+    const double2 h0 = *reinterpret_cast<const double2*>(Xr), h1 = *reinterpret_cast<const double2*>(Xr + 2);
+    const double2 xa = *reinterpret_cast<const double2*>(Xr + 4), xb = *reinterpret_cast<const double2*>(Xr + 6);
+    w.start(h0.y); w.warm1(h1.x); w.warm2(h1.y);
     w.warm3(xa.x);
     w.push(xa.y);
     w.push(xb.x);
-    const double F0 = spt_face(w, q.f0);
+    const double F0 = spt_face(w, f0);
     w.push(xb.y);
-    double Fprev = spt_face(w, q.f1);
+    double Fprev = spt_face(w, f1);
     double pend = fma(Fprev - F0, nrd, 0.0);                    // zone 0, stored with zone 1
 #pragma unroll 1
-    for (int it = 1; it <= 3; ++it) {
+    for (int it = 1; it <= 3; ++it) {                 // positions 4it .. 4it+3: faces 4it-2 .., zones 4it-3 ..
         double fc[4];
-        q.advance(fm, it, fc, keep);
-        const double2 xc = *reinterpret_cast<const double2*>(Xp + 4 * it), xd = *reinterpret_cast<const double2*>(Xp + 4 * it + 2);
-        double* __restrict__ pg = Pp + 4 * it - 4;                 // zones 4it-4 .. 4it-1 complete in this group
+#pragma unroll
+        for (int e = 0; e < 4; ++e) {
+            fc[e] = fn[e];
+            fn[e] = fnn[e];
+            if (it < 2 || (it == 2 && e < 3)) fnn[e] = spt_ldg(fm + (4 * it + 6 + e) * NTHR, keep);
+        }
+        const double2 xc = *reinterpret_cast<const double2*>(Xr + 4 + 4 * it), xd = *reinterpret_cast<const double2*>(Xr + 6 + 4 * it);
+        double* __restrict__ pg = Pp + 4 * it - 4;                 // zones 4it-4 .. 4it-1 are complete after this group
         double F, z, hold;
         w.push(xc.x); F = spt_face(w, fc[0]); z = fma(F - Fprev, nrd, 0.0); Fprev = F;
         *reinterpret_cast<double2*>(pg) = make_double2(pend, z);
@@ -195,11 +209,12 @@ __device__ __forceinline__ void spt_sweep_x(const double* __restrict__ Xp, doubl
         w.push(xd.y); F = spt_face(w, fc[3]); pend = fma(F - Fprev, nrd, 0.0); Fprev = F;
     }
     {
+        const double2 xe = *reinterpret_cast<const double2*>(Xr + 20), xf = *reinterpret_cast<const double2*>(Xr + 22);
         double F, z, hold;
-        w.push(hx[3]); F = spt_face(w, q.fn[0]); z = fma(F - Fprev, nrd, 0.0); Fprev = F;
+        w.push(xe.x); F = spt_face(w, fn[0]); z = fma(F - Fprev, nrd, 0.0); Fprev = F;
         *reinterpret_cast<double2*>(Pp + 12) = make_double2(pend, z);
-        w.push(hx[4]); F = spt_face(w, q.fn[1]); hold = fma(F - Fprev, nrd, 0.0); Fprev = F;
-        w.push(hx[5]); F = spt_face(w, q.fn[2]); z = fma(F - Fprev, nrd, 0.0);
+        w.push(xe.y); F = spt_face(w, fn[1]); hold = fma(F - Fprev, nrd, 0.0); Fprev = F;
+        w.push(xf.x); F = spt_face(w, fn[2]); z = fma(F - Fprev, nrd, 0.0);
         *reinterpret_cast<double2*>(Pp + 14) = make_double2(hold, z);
     }
 }
@@ -257,25 +272,35 @@ __device__ __forceinline__ void spt_write_out(const Geom& g, const TileCoord& tc
     }
 }
 
-// X = rho X / rho in place on the tile the TMA load has just delivered (waits for it on the mbarrier)
+// X = rho X / rho in place on the tile the TMA load has just delivered (waits for it on the mbarrier), x-halo columns
+// included.  A k plane of the tile is 16 rows x 24 columns = 384 consecutive doubles of shared memory: thread t takes
+// elements t (and t + 256 when below 384) of every plane; its (row, column) is the same in all 16 planes, and
+// consecutive threads read consecutive zones of a row of 1/rho.
 __device__ __forceinline__ void spt_convert(const Geom& g, const TileCoord& tc, double* __restrict__ Xs,
                                             const double* __restrict__ rinv_b, uint64_t* bar, const uint32_t parity,
                                             const unsigned long long keep)
 {
     const int ng = CST_NG;
-    const int tid = threadIdx.x, cp = tid & 7, r0 = tid >> 3;
-    const long long zrow = ((long long)(tc.k0 + ng + (r0 >> 4)) * g.ey + (tc.j0 + ng + (r0 & 15))) * g.ex + (tc.i0 + ng) + 2 * cp;
-    const double* pr = rinv_b + zrow;
-    double2 ri[8];
+    const int tid = threadIdx.x;
+    const long long zt = ((long long)(tc.k0 + ng) * g.ey + (tc.j0 + ng)) * g.ex + (tc.i0 + ng) - 4;
+    const int j1 = tid / SPT_XW, c1 = tid - j1 * SPT_XW;
+    const int e2 = tid + NTHR, j2 = e2 / SPT_XW, c2 = e2 - j2 * SPT_XW;
+    const bool two = e2 < SPT_XPLANE;
+    const double* p1 = rinv_b + zt + (long long)j1 * g.ex + c1;
+    const double* p2 = rinv_b + zt + (long long)j2 * g.ex + c2;
+    double r1[TILE], r2[TILE];
 #pragma unroll
-    for (int n = 0; n < 8; ++n) { ri[n] = spt_ldg2(pr, keep); pr += 2 * g.plane_g; }
+    for (int k = 0; k < TILE; ++k) r1[k] = spt_ldg(p1 + k * g.plane_g, keep);
+    if (two) {
+#pragma unroll
+        for (int k = 0; k < TILE; ++k) r2[k] = spt_ldg(p2 + k * g.plane_g, keep);
+    }
     mbar_wait(bar, parity);
-    double* x = Xs + r0 * SPT_PITCH + 2 * cp;
 #pragma unroll
-    for (int n = 0; n < 8; ++n) {
-        double2 v = *reinterpret_cast<const double2*>(x + 32 * n * SPT_PITCH);
-        v.x *= ri[n].x; v.y *= ri[n].y;
-        *reinterpret_cast<double2*>(x + 32 * n * SPT_PITCH) = v;
+    for (int k = 0; k < TILE; ++k) Xs[k * SPT_XPLANE + tid] *= r1[k];
+    if (two) {
+#pragma unroll
+        for (int k = 0; k < TILE; ++k) Xs[k * SPT_XPLANE + e2] *= r2[k];
     }
 }
 
@@ -287,18 +312,18 @@ __device__ __forceinline__ void spt_tile(const Geom& g, const TileCoord& tc, con
                                          double* __restrict__ sm, const int s_begin, const int s_end)
 {
     const int ng = CST_NG;
-    double* XB = sm;                                  // [2][SPT_TILE]
-    double* PB = sm + 2 * SPT_TILE;                   // [SPT_TILE]
-    uint64_t* bar = reinterpret_cast<uint64_t*>(sm + 3 * SPT_TILE);
+    double* Xs = sm;                                  // [SPT_XTILE]
+    double* PB = sm + SPT_XTILE;                      // [SPT_TILE]
+    uint64_t* bar = reinterpret_cast<uint64_t*>(sm + SPT_XTILE + SPT_TILE);
     const int tid = threadIdx.x, a = tid & (TILE - 1), b = tid >> 4;
-    const int zc0 = (tc.b * g.nvar) * g.ez + tc.k0 + ng;      // z coordinate of component 0 in the U tensor map
+    const int tx = tc.i0 + ng - 4, ty = tc.j0 + ng;           // x, y coordinates of the tile box in the U tensor map
+    const int zc0 = (tc.b * g.nvar) * g.ez + tc.k0 + ng;      // z coordinate of component 0
     const int za0 = (tc.b * g.nvar) * g.nz + tc.k0;           // ... in the A-like tensor maps
     if (tid == 0) {
-        mbar_init(&bar[0], 1);
-        mbar_init(&bar[1], 1);
+        mbar_init(bar, 1);
         fence_mbar_init();
-        mbar_expect_tx(&bar[0], SPT_TILE_BYTES);
-        tma_load_3d(XB, &maps.u, tc.i0 + ng, tc.j0 + ng, zc0 + (5 + s_begin) * g.ez, &bar[0]);
+        mbar_expect_tx(bar, SPT_XTILE_BYTES);
+        tma_load_3d(Xs, &maps.u, tx, ty, zc0 + (5 + s_begin) * g.ez, bar);
         // the tile's face mass fluxes and 1/rho star: one trip from HBM into L2 for all species passes
         bulk_prefetch_l2(fm_tile, 3 * (TILE + 1) * NTHR * 8);
         tma_prefetch_3d(&maps.r, tc.i0, tc.j0 + 1, tc.b * g.ez + tc.k0 + 1);
@@ -309,49 +334,43 @@ __device__ __forceinline__ void spt_tile(const Geom& g, const TileCoord& tc, con
     int n = 0;
 #pragma unroll 1
     for (int s = s_begin; s < s_end; ++s, ++n) {
-        const int c = 5 + s, cur = n & 1;
+        const int c = 5 + s;
         const bool last = (s + 1 >= s_end);
         // 1/rho and Fm of this tile stay in L2 (evict_last) until the last species, which demotes them
         const unsigned long long keep = last ? spt_policy_stream() : spt_policy_keep();
-        double* Xs = XB + cur * SPT_TILE;
         const double* Us = Ub + (long long)c * g.comp_g;
-        if (n > 0) {
-            __syncthreads();                          // z sweep of the previous species done: P complete
-            spt_write_out<NR>(g, tc, PB, A, up, c - 1);
-        }
-        spt_convert(g, tc, Xs, rinv_b, &bar[cur], (n >> 1) & 1, keep);
-        SptHalo hr;
-        spt_halo_load(g, tc, 0, Us, rinv_b, hr, keep);
-        __syncthreads();                              // X complete; P and the other X buffer are free
-        if (tid == 0) {
-            if (!last) {
-                fence_proxy_async();
-                mbar_expect_tx(&bar[cur ^ 1], SPT_TILE_BYTES);
-                tma_load_3d(XB + (cur ^ 1) * SPT_TILE, &maps.u, tc.i0 + ng, tc.j0 + ng, zc0 + (c + 1) * g.ez, &bar[cur ^ 1]);
-            }
-            if (NR > 0) {                             // operands of this species' write-out: into L2 a pass ahead
+        if (n > 0) spt_write_out<NR>(g, tc, PB, A, up, c - 1);       // overlaps the tile load issued after the z sweep
+        if (tid == 0) {                               // L2 prefetches a pass ahead: next species' tile, this species' write-out operands
+            if (!last) tma_prefetch_3d(&maps.u, tx, ty, zc0 + (c + 1) * g.ez);
+            if (NR > 0) {
 #pragma unroll
                 for (int r = 0; r < NR; ++r) tma_prefetch_3d(&maps.p[r], tc.i0, tc.j0, za0 + c * g.nz);
             }
         }
+        spt_convert(g, tc, Xs, rinv_b, bar, n & 1, keep);
+        SptHalo hr;
+        spt_halo_load(g, tc, 1, Us, rinv_b, hr, keep);           // operands of the y sweep: in flight during the x sweep
+        __syncthreads();                              // X complete; P free (written out)
         double hx[6];
         // ---- x sweep
-#pragma unroll
-        for (int m = 0; m < 6; ++m) hx[m] = hr.u[m] * hr.r[m];
-        spt_halo_load(g, tc, 1, Us, rinv_b, hr, keep);          // operands of the y sweep: in flight during the x sweep
-        spt_sweep_x(Xs + spt_sbase<0>(a, b), PB + spt_sbase<0>(a, b), fm, hx, nrdx, keep);
+        spt_sweep_x(Xs + spt_xbase<0>(a, b), PB + spt_pbase<0>(a, b), fm, nrdx, keep);
         __syncthreads();
         // ---- y sweep
 #pragma unroll
         for (int m = 0; m < 6; ++m) hx[m] = hr.u[m] * hr.r[m];
         spt_halo_load(g, tc, 2, Us, rinv_b, hr, keep);
-        spt_sweep_yz<1>(Xs + spt_sbase<1>(a, b), PB + spt_sbase<1>(a, b), fm + (TILE + 1) * NTHR, hx, nrdy, keep);
+        spt_sweep_yz<1>(Xs + spt_xbase<1>(a, b), PB + spt_pbase<1>(a, b), fm + (TILE + 1) * NTHR, hx, nrdy, keep);
         __syncthreads();
         // ---- z sweep
 #pragma unroll
         for (int m = 0; m < 6; ++m) hx[m] = hr.u[m] * hr.r[m];
-        spt_sweep_yz<2>(Xs + spt_sbase<2>(a, b), PB + spt_sbase<2>(a, b), fm + 2 * (TILE + 1) * NTHR, hx, nrdz, keep);
+        spt_sweep_yz<2>(Xs + spt_xbase<2>(a, b), PB + spt_pbase<2>(a, b), fm + 2 * (TILE + 1) * NTHR, hx, nrdz, keep);
+        __syncthreads();                              // X released, P complete
+        if (tid == 0 && !last) {                      // next species' tile (already in L2): lands during the write-out
+            fence_proxy_async();
+            mbar_expect_tx(bar, SPT_XTILE_BYTES);
+            tma_load_3d(Xs, &maps.u, tx, ty, zc0 + (c + 1) * g.ez, bar);
+        }
     }
-    __syncthreads();
     spt_write_out<NR>(g, tc, PB, A, up, 5 + s_end - 1);
 }
