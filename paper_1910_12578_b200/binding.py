@@ -8,7 +8,7 @@ import ctypes as C
 import os
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libcst.so")
+LIB_PATH = os.environ.get("CST_LIB_PATH") or os.path.join(_HERE, "libcst.so")   # override: A/B builds while tuning
 MAX_QUAD = 4
 
 EXPORTS = ["cst_create", "cst_destroy", "cst_workspace_bytes", "cst_set_workspace", "cst_fill_ghosts", "cst_advance_A", "cst_sdc_update",
