@@ -416,10 +416,14 @@ def main():
         import gc
         gc.collect()
         torch.cuda.empty_cache()
-        also = measure(wl.make_config(4), args, rank, world, local, dev, False, False)
-        if rank == 0:
-            keep = ("value", "unit", "ms_per_step", "steps", "warmup", "config", "clocks", "gpu_launches", "roofline")
-            line["also"] = {"configs[4]": {k: also[k] for k in keep}}
+        try:
+            also = measure(wl.make_config(4), args, rank, world, local, dev, False, False)
+            if rank == 0:
+                keep = ("value", "unit", "ms_per_step", "steps", "warmup", "config", "clocks", "gpu_launches", "roofline")
+                line["also"] = {"configs[4]": {k: also[k] for k in keep}}
+        except Exception as exc:    # the headline line must still be printed
+            if rank == 0:
+                line["also"] = {"configs[4]": {"error": f"{type(exc).__name__}: {exc}"}}
     if rank == 0:
         print(json.dumps(line), flush=True)
     if world > 1:
