@@ -10,8 +10,11 @@ inside the same line under "also" (both halves of the north-star target get a nu
 --workload K times configs[K] only.  Prints ONE JSON line (rank 0).
 
   python bench.py [--gpus N] [--steps K] [--warmup W] [--workload 3|4] [--impl ours|reference]
-Multi-GPU: launched by torchrun, one rank per GPU; every rank runs the workload on its own
-replica of the domain (weak scaling, no data-path collective; dt is all-reduced with MIN).
+Multi-GPU (launched by torchrun, one rank per GPU): the box lattice is SHARDED over the ranks in equal bricks
+(strong scaling: the global domain is fixed; paper_1910_12578_b200/shard.py, csrc/exchange.cu).  configs[3]'s 512^3
+domain is then a 2 x 2 x 2 lattice of 256^3 boxes, configs[4] keeps its 16 x 8 x 4 boxes of 64^3.  Per step every rank
+fills its local ghost zones, exchanges the 4-deep shells on its brick surface with the neighbouring ranks
+(NCCL send/recv), advances its boxes and MIN-reduces dt; `value` = zones of the whole domain / max-over-ranks time.
 """
 import argparse
 import json
@@ -70,14 +73,16 @@ def measured_peaks():
 
 
 # ----------------------------------------------------------------------------------- inputs ----
-def fill_host_state(cfg, U_host_np, threads=8):
-    """Seeded synthetic state of the config, plane by plane, into the host array (ghosts zero)."""
+def fill_host_state(cfg, U_host_np, threads=8, brick=None):
+    """Seeded synthetic state of the config, plane by plane, into the host array (ghosts zero).  brick = (origin,
+    lattice) in box coordinates: only that rank's boxes (the planes are generated for the global domain)."""
     Dz = wl.domain(cfg)[2]
+    planes = range(Dz) if brick is None else range(brick[0][2] * cfg["nz"], (brick[0][2] + brick[1][2]) * cfg["nz"])
 
     def one(kg):
-        wl.scatter_plane(cfg, U_host_np, kg, wl.cons_plane(cfg, kg))
+        wl.scatter_plane(cfg, U_host_np, kg, wl.cons_plane(cfg, kg), brick)
     with ThreadPoolExecutor(threads) as ex:
-        list(ex.map(one, range(Dz)))
+        list(ex.map(one, planes))
 
 
 def host_mem_available():
@@ -202,8 +207,21 @@ def allreduce_scalar(x, op, device, world):
 
 
 def aggregate_value(zones_per_rank, world, ms_step_max):
-    """whole-job zone-updates/s: every rank advances its own zones_per_rank zones in ms_step_max."""
+    """whole-job zone-updates/s: every rank advances its own zones_per_rank zones (its brick of the sharded
+    lattice) in ms_step_max, the slowest rank's time."""
     return zones_per_rank * world / (ms_step_max * 1e-3)
+
+
+def sharded_config(cfg, world):
+    """The config a multi-rank run shards (same global domain and seeded state as the single-GPU workload) and its
+    partition into bricks.  configs[3]'s single 512^3 box becomes 2 x 2 x 2 boxes of 256^3 (a box is the unit of
+    distribution); the batched configs keep their lattice."""
+    from paper_1910_12578_b200 import shard
+    if cfg["nbx"] * cfg["nby"] * cfg["nbz"] == 1 and world > 1:
+        f = 2 if world <= 8 else 4
+        cfg = wl.make_config(cfg["index"], n=(cfg["nx"] // f, cfg["ny"] // f, cfg["nz"] // f), nb=(f, f, f), nspec=cfg["nspec"])
+    part = shard.brick_partition((cfg["nbx"], cfg["nby"], cfg["nbz"]), world)
+    return cfg, part
 
 
 # -------------------------------------------------------------------------------------- main ----
@@ -214,6 +232,14 @@ def measure(cfg, args, rank, world, local, dev, want_e2e, want_cpu_baseline):
     import torch.distributed as dist
     from paper_1910_12578_b200 import Context
 
+    from paper_1910_12578_b200 import shard
+    gcfg, part, brick = cfg, (1, 1, 1), None          # gcfg: the global lattice; cfg: this rank's brick of it
+    if world > 1:
+        gcfg, part = sharded_config(cfg, world)
+        cfg = shard.local_config(gcfg, part)
+        pc = shard.rank_coords(part, rank)
+        lat = (cfg["nbx"], cfg["nby"], cfg["nbz"])
+        brick = (tuple(pc[d] * lat[d] for d in range(3)), lat)
     ctx = Context(cfg)
     ctx_sm_count = torch.cuda.get_device_properties(dev).multi_processor_count
     N, zones = wl.nvar(cfg), wl.nzones(cfg)
@@ -227,7 +253,7 @@ def measure(cfg, args, rank, world, local, dev, want_e2e, want_cpu_baseline):
     except Exception:
         pinned = False
         U_host = torch.zeros(ushape, dtype=torch.float64)
-    fill_host_state(cfg, U_host.numpy())
+    fill_host_state(gcfg, U_host.numpy(), brick=brick)
 
     U = torch.empty(ushape, dtype=torch.float64, device=dev)
     U.copy_(U_host, non_blocking=True)
@@ -236,7 +262,11 @@ def measure(cfg, args, rank, world, local, dev, want_e2e, want_cpu_baseline):
     A_old0 = torch.zeros(ashape, dtype=torch.float64, device=dev)
     A_old1 = torch.zeros(ashape, dtype=torch.float64, device=dev)
     dt_dev = torch.zeros(1, dtype=torch.float64, device=dev)
-    ctx.fill_ghosts(U)
+    ex = None
+    if world > 1:                 # ghost zones with a source on another rank travel through NCCL send/recv
+        ex = shard.GhostExchange(ctx, gcfg, part, rank, lambda n: torch.empty(n, dtype=torch.float64, device=dev))
+    fill = (lambda: ex.fill_ghosts(U)) if ex else (lambda: ctx.fill_ghosts(U))
+    fill()
     dt = ctx.cfl_dt(U, 0.5)
     dt = allreduce_scalar(dt, "min", dev, world)
     # A_old buffers hold plausible values: A of the initial state and a perturbation of it
@@ -253,7 +283,7 @@ def measure(cfg, args, rank, world, local, dev, want_e2e, want_cpu_baseline):
     def step(timed):
         if timed:
             step_ev.append(ev()); step_ev[-1].record()
-        ctx.fill_ghosts(U)
+        fill()
         if timed:
             e0, e1 = ev(), ev()
             e0.record()
@@ -262,6 +292,8 @@ def measure(cfg, args, rank, world, local, dev, want_e2e, want_cpu_baseline):
             e1.record()
             k_ev.append((e0, e1))
         ctx.cfl_dt_device(U, 0.5, dt_dev)
+        if world > 1:
+            dist.all_reduce(dt_dev, op=dist.ReduceOp.MIN)
 
     def sync_all():
         if world > 1:
@@ -352,17 +384,29 @@ def measure(cfg, args, rank, world, local, dev, want_e2e, want_cpu_baseline):
             A_host = torch.empty(ashape, dtype=torch.float64)
             Un_host = torch.empty(ushape, dtype=torch.float64)
         n_e2e = max(1, min(args.steps, 2))
-        ctx.step_host(U_host, A_host, Un_host, U, U_next, A_new, dt)       # warm-up
+
+        def host_step():
+            if ex is None:                  # one C-ABI call with HOST buffers
+                ctx.step_host(U_host, A_host, Un_host, U, U_next, A_new, dt)
+            else:                           # sharded: the same sequence with the ghost exchange between H2D and the advance
+                U.copy_(U_host, non_blocking=True)
+                ex.fill_ghosts(U)
+                ctx.advance_A_update(U, A_new, U_next, dt, A_new, [A_new, A_new], w)
+                A_host.copy_(A_new, non_blocking=True)
+                Un_host.copy_(U_next, non_blocking=True)
+                torch.cuda.synchronize()
+        host_step()                         # warm-up
         sync_all()
         t0 = time.perf_counter()
         for _ in range(n_e2e):
-            ctx.step_host(U_host, A_host, Un_host, U, U_next, A_new, dt)
+            host_step()
         sync_all()
         sec = (time.perf_counter() - t0) / n_e2e
         sec = allreduce_scalar(sec, "max", dev, world)
-        e2e = {"value": zones * world / sec, "unit": UNIT, "h2d_bytes_per_step": ubytes,
-               "d2h_bytes_per_step": abytes + ubytes, "steps": n_e2e, "host_memory": "pinned" if pinned else "pageable",
-               "call": "cst_step_host (H2D U, fill_ghosts, advance_A_update, D2H A and U_next)"}
+        e2e = {"value": zones * world / sec, "unit": UNIT, "h2d_bytes_per_step": ubytes * world,
+               "d2h_bytes_per_step": (abytes + ubytes) * world, "steps": n_e2e, "host_memory": "pinned" if pinned else "pageable",
+               "call": "cst_step_host (H2D U, fill_ghosts, advance_A_update, D2H A and U_next)" if ex is None else
+                       "H2D U, fill_ghosts + ghost exchange, cst_advance_A_update, D2H A and U_next (per rank, its brick)"}
         del A_host, Un_host
 
     cpu_baseline = None
@@ -372,14 +416,19 @@ def measure(cfg, args, rank, world, local, dev, want_e2e, want_cpu_baseline):
     line = None
     if rank == 0:
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-                "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
+                "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "strong",
                 "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-                "config": {"workload": f"configs[{cfg['index']}] {cfg['name']}: {cfg['nbx'] * cfg['nby'] * cfg['nbz']} box(es) of "
-                                       f"{cfg['nx']}x{cfg['ny']}x{cfg['nz']}+{cfg['ng']} ghosts, NVAR={N}",
-                           "zones_per_gpu": zones, "step": "fill_ghosts + advance_A_update + cfl_dt_device",
+                "config": {"workload": f"configs[{gcfg['index']}] {gcfg['name']}: {gcfg['nbx'] * gcfg['nby'] * gcfg['nbz']} box(es) of "
+                                       f"{gcfg['nx']}x{gcfg['ny']}x{gcfg['nz']}+{gcfg['ng']} ghosts, NVAR={N}",
+                           "zones_per_gpu": zones, "zones_total": zones * world,
+                           "step": "fill_ghosts + advance_A_update + cfl_dt_device" if ex is None else
+                                   "fill_ghosts + exchange_pack + NCCL send/recv + exchange_unpack + advance_A_update + "
+                                   "cfl_dt_device + all_reduce(MIN) of dt",
+                           "ghost_exchange_bytes_per_rank_per_step": ex.bytes_per_fill if ex else 0,
                            "l2": f"inputs larger than L2 ({(ubytes + 3 * abytes) / 1e9:.1f} GB touched per step)"
                                  if ubytes > 4e8 else "inputs fit in L2 (debug size)",
-                           "parallelism": f"replicas x{world}" if world > 1 else "single GPU",
+                           "parallelism": f"box lattice sharded over {world} ranks, bricks {part[0]}x{part[1]}x{part[2]}" if world > 1
+                                          else "single GPU",
                            "ms_per_step_best": float(min(per_step)), "ms_per_step_median": float(np.median(per_step)),
                            "debug_size_override": bool(args.n)},
                 "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline,

@@ -76,6 +76,41 @@ int cst_set_workspace(cst_ctx* ctx, void* workspace_dev, long long bytes);
  * wall-normal momentum negated.  Interior zones are not touched. */
 int cst_fill_ghosts(cst_ctx* ctx, double* U, void* stream);
 
+/* Box lattice sharded over ranks ("MPI distribute the AMR grids across nodes").
+ * The global lattice of global_nb[0] x [1] x [2] boxes is cut into part[0] x part[1] x part[2] equal bricks, brick
+ * (pi, pj, pk) owned by rank pi + part[0]*(pj + part[1]*pk); global_nb[d] must be a multiple of part[d].
+ * cst_set_sublattice declares that the context (created with nbx, nby, nbz = the BRICK's lattice; bc_lo / bc_hi = the
+ * boundaries of the GLOBAL domain) holds the brick of `rank`.  From then on cst_fill_ghosts uses the global zone map
+ * and fills every ghost zone whose source box is local; the others arrive from the neighbouring ranks:
+ *   cst_exchange_pack   writes, for every peer, one message (the source zones of all the peer's ghost regions that
+ *                       read this brick, in the peer's zone order, reflecting-wall signs applied) into sendbuf;
+ *   [the caller moves sendbuf[send_off[p] .. +send_len[p]) to peer p's recvbuf[recv_off .. +recv_len): NCCL / MPI]
+ *   cst_exchange_unpack copies the received messages into the ghost regions of U.
+ * cst_exchange_info: number of peers (<= 26) and, per peer (ascending rank), offsets and lengths in DOUBLES of its
+ * message inside the send / receive buffers (DEVICE buffers owned by the caller, at least sum(len) doubles).
+ * Every other call works on the local boxes unchanged; the time step needs a MIN over ranks of cst_cfl_dt.
+ * CST_EINVAL: lattice not divisible, brick != the context's lattice, rank out of range, no plan set.
+ *
+ * cst_exchange_plan is the plan itself as a pure HOST function (no GPU, no context): the segments of `rank`
+ * (recv = 1: its ghost regions with a remote source; recv = 0: what it sends), grouped by peer in ascending order.
+ * `global` describes the GLOBAL lattice.  Returns the number of segments (call with segs = NULL to size the array). */
+typedef struct {
+    int peer;              /* rank on the other side                                                        */
+    int box;               /* LOCAL box index on this side: source box (send) or destination box (recv)      */
+    int lo[3];             /* ghosted (i, j, k) index of the first zone on this side                         */
+    int step[3];           /* send: +1 neighbour / periodic, 0 outflow, -1 reflecting mirror; recv: +1        */
+    int ext[3];            /* zones per direction (extents of the destination region)                        */
+    int flip[3];           /* send: 1 = the momentum component along d changes sign (reflecting wall)        */
+    long long offset;      /* doubles from the start of this peer's message; segment data is [c][k][j][i]    */
+} cst_xseg;
+long long cst_exchange_plan(const cst_params* global, const int part[3], int rank, int recv,
+                            cst_xseg* segs, long long cap);
+int cst_set_sublattice(cst_ctx* ctx, const int global_nb[3], const int part[3], int rank);
+int cst_exchange_info(const cst_ctx* ctx, int* npeers, int* peers, long long* send_off, long long* send_len,
+                      long long* recv_off, long long* recv_len, int cap);
+int cst_exchange_pack(cst_ctx* ctx, const double* U, double* sendbuf, void* stream);
+int cst_exchange_unpack(cst_ctx* ctx, double* U, const double* recvbuf, void* stream);
+
 /* S1-S4.  A <- <A(U)>: conserved->primitive with the gamma-law EOS, PPM
  * reconstruction (Colella & Woodward 1984 limiter, P:L52 ref [15]) of the primitives in x, y, z,
  * an HLLC Riemann solve at every face, flux divergence plus the constant-gravity source.

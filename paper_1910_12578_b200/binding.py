@@ -14,7 +14,8 @@ MAX_QUAD = 4
 EXPORTS = ["cst_create", "cst_destroy", "cst_workspace_bytes", "cst_set_workspace", "cst_fill_ghosts", "cst_advance_A", "cst_sdc_update",
            "cst_advance_A_update", "cst_cfl_dt_device", "cst_cfl_dt", "cst_validate", "cst_step_host",
            "cst_set_timing", "cst_last_advance_ms", "cst_launch_count", "cst_strerror", "cst_version",
-           "cst_debug_rcp_sqrt", "cst_debug_tile_count", "cst_debug_tile_map"]
+           "cst_debug_rcp_sqrt", "cst_debug_tile_count", "cst_debug_tile_map",
+           "cst_exchange_plan", "cst_set_sublattice", "cst_exchange_info", "cst_exchange_pack", "cst_exchange_unpack"]
 
 
 class CstParams(C.Structure):
@@ -24,6 +25,12 @@ class CstParams(C.Structure):
                 ("gamma", C.c_double), ("grav", C.c_double * 3),
                 ("bc_lo", C.c_int * 3), ("bc_hi", C.c_int * 3),
                 ("small_dens", C.c_double), ("small_pres", C.c_double)]
+
+
+class CstXseg(C.Structure):
+    """cst_xseg of include/cst.h: one ghost region that crosses ranks."""
+    _fields_ = [("peer", C.c_int), ("box", C.c_int), ("lo", C.c_int * 3), ("step", C.c_int * 3),
+                ("ext", C.c_int * 3), ("flip", C.c_int * 3), ("offset", C.c_longlong)]
 
 
 class CstError(RuntimeError):
@@ -67,6 +74,13 @@ def load():
     lib.cst_debug_tile_map.argtypes = [_vp, _vp, _vp]
     lib.cst_launch_count.argtypes = [_vp]
     lib.cst_launch_count.restype = C.c_longlong
+    I3, LLP = C.POINTER(C.c_int), C.POINTER(C.c_longlong)
+    lib.cst_exchange_plan.argtypes = [P, I3, C.c_int, C.c_int, C.POINTER(CstXseg), C.c_longlong]
+    lib.cst_exchange_plan.restype = C.c_longlong
+    lib.cst_set_sublattice.argtypes = [_vp, I3, I3, C.c_int]
+    lib.cst_exchange_info.argtypes = [_vp, I3, I3, LLP, LLP, LLP, LLP, C.c_int]
+    lib.cst_exchange_pack.argtypes = [_vp, _vp, _vp, _vp]
+    lib.cst_exchange_unpack.argtypes = [_vp, _vp, _vp, _vp]
     lib.cst_strerror.argtypes = [C.c_int]
     lib.cst_strerror.restype = C.c_char_p
     lib.cst_version.restype = C.c_char_p
@@ -85,6 +99,20 @@ def make_params(cfg) -> CstParams:
         p.bc_lo[d] = int(cfg["bc_lo"][d])
         p.bc_hi[d] = int(cfg["bc_hi"][d])
     return p
+
+
+def exchange_plan(cfg_global, part, rank, recv):
+    """cst_exchange_plan (pure host function, needs no GPU): the list of CstXseg of `rank` for the GLOBAL lattice
+    described by cfg_global cut into part[0] x part[1] x part[2] bricks."""
+    lib = load()
+    p = make_params(cfg_global)
+    pa = (C.c_int * 3)(*[int(x) for x in part])
+    n = lib.cst_exchange_plan(C.byref(p), pa, int(rank), int(bool(recv)), None, 0)
+    if n < 0:
+        raise CstError(n, "cst_exchange_plan", lib.cst_strerror(int(n)).decode())
+    segs = (CstXseg * max(int(n), 1))()
+    lib.cst_exchange_plan(C.byref(p), pa, int(rank), int(bool(recv)), segs, n)
+    return [segs[i] for i in range(int(n))]
 
 
 def _ptr(t):
@@ -189,6 +217,27 @@ class Context:
         self._check(self.lib.cst_step_host(self._h, _ptr(U_host), _ptr(A_host), _ptr(U_next_host), _ptr(U_dev),
                                            _ptr(U_next_dev), _ptr(A_dev), float(dt_m), _stream(stream)),
                     "cst_step_host")
+
+    def set_sublattice(self, global_nb, part, rank):
+        g = (C.c_int * 3)(*[int(x) for x in global_nb])
+        p = (C.c_int * 3)(*[int(x) for x in part])
+        self._check(self.lib.cst_set_sublattice(self._h, g, p, int(rank)), "cst_set_sublattice")
+
+    def exchange_info(self):
+        """-> list of (peer, send_off, send_len, recv_off, recv_len), offsets / lengths in doubles."""
+        cap = 32
+        n = C.c_int(0)
+        peers = (C.c_int * cap)()
+        arr = [(C.c_longlong * cap)() for _ in range(4)]
+        self._check(self.lib.cst_exchange_info(self._h, C.byref(n), peers, arr[0], arr[1], arr[2], arr[3], cap),
+                    "cst_exchange_info")
+        return [(peers[i], arr[0][i], arr[1][i], arr[2][i], arr[3][i]) for i in range(n.value)]
+
+    def exchange_pack(self, U, sendbuf, stream=None):
+        self._check(self.lib.cst_exchange_pack(self._h, _ptr(U), _ptr(sendbuf), _stream(stream)), "cst_exchange_pack")
+
+    def exchange_unpack(self, U, recvbuf, stream=None):
+        self._check(self.lib.cst_exchange_unpack(self._h, _ptr(U), _ptr(recvbuf), _stream(stream)), "cst_exchange_unpack")
 
     def set_timing(self, on):
         self._check(self.lib.cst_set_timing(self._h, int(bool(on))), "cst_set_timing")

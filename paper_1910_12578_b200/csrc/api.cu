@@ -47,6 +47,7 @@ extern "C" int cst_create(const cst_params* p, cst_ctx** out)
     g.nx = p->nx; g.ny = p->ny; g.nz = p->nz;
     g.ex = p->nx + 2 * CST_NG; g.ey = p->ny + 2 * CST_NG; g.ez = p->nz + 2 * CST_NG;
     g.nbx = p->nbx; g.nby = p->nby; g.nbz = p->nbz; g.nbox = p->nbx * p->nby * p->nbz;
+    g.gnbx = p->nbx; g.gnby = p->nby; g.gnbz = p->nbz; g.obx = g.oby = g.obz = 0;   // the whole lattice is local
     g.nspec = p->nspec; g.nvar = 5 + p->nspec;
     for (int d = 0; d < 3; ++d) { g.bc_lo[d] = p->bc_lo[d]; g.bc_hi[d] = p->bc_hi[d]; g.grav[d] = p->grav[d]; }
     g.dx = p->dx; g.dy = p->dy; g.dz = p->dz;
@@ -62,6 +63,7 @@ extern "C" int cst_create(const cst_params* p, cst_ctx** out)
     c->launches = 0;
     c->ws = nullptr; c->ws_bytes = 0;
     c->timing = 0;
+    c->xplan = nullptr;
     for (int n = 0; n < 3; ++n) c->ev[n] = nullptr;
     int dev = 0;
     cudaError_t e = cudaGetDevice(&dev);
@@ -75,6 +77,7 @@ extern "C" int cst_create(const cst_params* p, cst_ctx** out)
 extern "C" int cst_destroy(cst_ctx* c)
 {
     if (!c) return CST_EINVAL;
+    xplan_destroy(c);
     cudaFree(c->d_scratch);
     for (int n = 0; n < 3; ++n) if (c->ev[n]) cudaEventDestroy(c->ev[n]);
     delete c;
@@ -206,6 +209,32 @@ extern "C" int cst_step_host(cst_ctx* c, const double* U_host, double* A_host, d
     if (e == cudaSuccess) e = cudaMemcpyAsync(U_next_host, U_next_dev, ub, cudaMemcpyDeviceToHost, st);
     if (e == cudaSuccess) e = cudaStreamSynchronize(st);
     return e == cudaSuccess ? CST_OK : cuda_fail(e);
+}
+
+extern "C" int cst_set_sublattice(cst_ctx* c, const int global_nb[3], const int part[3], int rank)
+{
+    if (!c || !global_nb || !part) return CST_EINVAL;
+    const int rc = xplan_create(c, global_nb, part, rank);
+    return rc == CST_ECUDA ? cuda_fail(cudaGetLastError()) : rc;
+}
+
+extern "C" int cst_exchange_info(const cst_ctx* c, int* npeers, int* peers, long long* send_off, long long* send_len,
+                                 long long* recv_off, long long* recv_len, int cap)
+{
+    if (!c) return CST_EINVAL;
+    return xplan_info(c, npeers, peers, send_off, send_len, recv_off, recv_len, cap);
+}
+
+extern "C" int cst_exchange_pack(cst_ctx* c, const double* U, double* sendbuf, void* stream)
+{
+    if (!c || !U || !sendbuf) return CST_EINVAL;
+    return check_launch(launch_exchange_pack(c, U, sendbuf, (cudaStream_t)stream));
+}
+
+extern "C" int cst_exchange_unpack(cst_ctx* c, double* U, const double* recvbuf, void* stream)
+{
+    if (!c || !U || !recvbuf) return CST_EINVAL;
+    return check_launch(launch_exchange_unpack(c, U, recvbuf, (cudaStream_t)stream));
 }
 
 extern "C" int cst_set_timing(cst_ctx* c, int on)

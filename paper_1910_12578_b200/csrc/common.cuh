@@ -11,6 +11,8 @@ struct Geom {
     int nx, ny, nz;          // interior zones per box
     int ex, ey, ez;          // ghosted extents
     int nbx, nby, nbz, nbox;
+    int gnbx, gnby, gnbz;    // global box lattice this context's boxes are a brick of (cst_set_sublattice; default = local)
+    int obx, oby, obz;       // lattice coordinates of local box (0, 0, 0) in the global lattice
     int nspec, nvar;
     int bc_lo[3], bc_hi[3];
     double dx, dy, dz;
@@ -35,6 +37,7 @@ struct cst_ctx {
     int sm_count;
     int timing;              // cst_set_timing: record events around the kernels of the advance calls
     cudaEvent_t ev[3];       // before hydro, between hydro and species, after species
+    struct XPlan* xplan;     // cst_set_sublattice: ghost-exchange plan with the neighbouring ranks (exchange.cu)
 };
 
 struct UpdArgs;
@@ -64,6 +67,13 @@ int launch_sdc_update(cst_ctx*, double* U_next, const double* U_m, double dt_m,
                       const double* A_new_m, const double* A_old_m, const QuadArgs& q, cudaStream_t);
 int launch_cfl(cst_ctx*, const double* U, double cfl, double* dt_out_dev, cudaStream_t);
 int launch_validate(cst_ctx*, const double* U, cudaStream_t);   // count left in d_scratch[2]
+// exchange.cu: box lattice sharded over ranks
+int xplan_create(cst_ctx*, const int global_nb[3], const int part[3], int rank);
+void xplan_destroy(cst_ctx*);
+int xplan_info(const cst_ctx*, int* npeers, int* peers, long long* send_off, long long* send_len,
+               long long* recv_off, long long* recv_len, int cap);
+int launch_exchange_pack(cst_ctx*, const double* U, double* sendbuf, cudaStream_t);
+int launch_exchange_unpack(cst_ctx*, double* U, const double* recvbuf, cudaStream_t);
 int launch_debug_rcp_sqrt(const double* x, double* r, double* s, long long n, cudaStream_t);
 long long debug_tile_count(const Geom& g);
 int launch_debug_tile_map(cst_ctx*, int* out, cudaStream_t);

@@ -2,6 +2,8 @@
 // One thread per ghost zone (all components); ghost zones are enumerated region by region
 // (z slabs, then y slabs, then x slabs) so that no thread is spent on interior zones.
 // Sources are always interior zones, so the in-place fill has no ordering hazard.
+// When the context's boxes are a brick of a larger lattice (cst_set_sublattice, exchange.cu) the zone map is the
+// GLOBAL one; ghost zones whose source box lives on another rank are left for cst_exchange_unpack.
 #include "common.cuh"
 
 __device__ __forceinline__ int map_dir(int g, int D, int bc_lo, int bc_hi, bool& flip)
@@ -53,13 +55,15 @@ k_fill_ghosts(Geom g, double* __restrict__ U, long long n0, long long n1, long l
         i = ii < ng ? ii : ii + g.nx;
     }
     bool fx, fy, fz;
-    const int sx = map_dir(bi * g.nx + i - ng, g.nbx * g.nx, g.bc_lo[0], g.bc_hi[0], fx);
-    const int sy = map_dir(bj * g.ny + j - ng, g.nby * g.ny, g.bc_lo[1], g.bc_hi[1], fy);
-    const int sz = map_dir(bk * g.nz + k - ng, g.nbz * g.nz, g.bc_lo[2], g.bc_hi[2], fz);
-    const int sbi = sx / g.nx, sbj = sy / g.ny, sbk = sz / g.nz;
+    const int sx = map_dir((bi + g.obx) * g.nx + i - ng, g.gnbx * g.nx, g.bc_lo[0], g.bc_hi[0], fx);
+    const int sy = map_dir((bj + g.oby) * g.ny + j - ng, g.gnby * g.ny, g.bc_lo[1], g.bc_hi[1], fy);
+    const int sz = map_dir((bk + g.obz) * g.nz + k - ng, g.gnbz * g.nz, g.bc_lo[2], g.bc_hi[2], fz);
+    const int gbi = sx / g.nx, gbj = sy / g.ny, gbk = sz / g.nz;          // source box in the global lattice
+    const int sbi = gbi - g.obx, sbj = gbj - g.oby, sbk = gbk - g.obz;    // ... in this rank's brick
+    if (sbi < 0 || sbi >= g.nbx || sbj < 0 || sbj >= g.nby || sbk < 0 || sbk >= g.nbz) return;   // remote source
     const int sb = sbi + g.nbx * (sbj + g.nby * sbk);
     // the zone map is the same for every component: one thread moves all NVAR values of its ghost zone
-    const double* __restrict__ src = U + uidx(g, sb, 0, sz - sbk * g.nz + ng, sy - sbj * g.ny + ng, sx - sbi * g.nx + ng);
+    const double* __restrict__ src = U + uidx(g, sb, 0, sz - gbk * g.nz + ng, sy - gbj * g.ny + ng, sx - gbi * g.nx + ng);
     double* __restrict__ dst = U + uidx(g, b, 0, k, j, i);
     const double s1 = fx ? -1.0 : 1.0, s2 = fy ? -1.0 : 1.0, s3 = fz ? -1.0 : 1.0;
     int c = 0;

@@ -148,14 +148,19 @@ def cons_plane(cfg, kg):
     return cons_from_prim(cfg, prim_plane(cfg, kg))
 
 
-def scatter_plane(cfg, Ubox, kg, plane):
+def scatter_plane(cfg, Ubox, kg, plane, brick=None):
     """Write global plane kg (array [N, Dy, Dx], numpy or torch) into the box-layout array
-    Ubox[b][c][k][j][i] (numpy or torch; ghosts untouched)."""
+    Ubox[b][c][k][j][i] (numpy or torch; ghosts untouched).  brick = (origin, lattice) of a rank's brick of the box
+    lattice (box coordinates; paper_1910_12578_b200/shard.py): Ubox then holds only that brick's boxes, in the
+    brick's local order, and planes outside it are ignored."""
     ng, nx, ny, nz = cfg["ng"], cfg["nx"], cfg["ny"], cfg["nz"]
+    (ox, oy, oz), (lx, ly, lz) = brick if brick is not None else ((0, 0, 0), (cfg["nbx"], cfg["nby"], cfg["nbz"]))
     bk, lk = divmod(int(kg), nz)
-    for bj in range(cfg["nby"]):
-        for bi in range(cfg["nbx"]):
-            b = bi + cfg["nbx"] * (bj + cfg["nby"] * bk)
+    if not (oz <= bk < oz + lz):
+        return
+    for bj in range(oy, oy + ly):
+        for bi in range(ox, ox + lx):
+            b = (bi - ox) + lx * ((bj - oy) + ly * (bk - oz))
             Ubox[b, :, lk + ng, ng:ng + ny, ng:ng + nx] = \
                 plane[:, bj * ny:(bj + 1) * ny, bi * nx:(bi + 1) * nx]
 

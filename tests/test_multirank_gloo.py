@@ -1,5 +1,7 @@
-"""The N > 1 path of bench.py on CPU: world_size 2, gloo.  The path shards as independent replicas
-(DESIGN.md section 9); the only cross-rank traffic is MIN of dt and MAX of the device time."""
+"""The N > 1 path of bench.py on CPU: world_size 2, gloo.  The box lattice is sharded over the ranks (DESIGN.md
+section 9): the scalar reductions (MIN of dt, MAX of the device time), the sharded workload and each rank's share of
+the seeded input are checked here; the ghost exchange itself in tests/test_shard_plan.py (gloo) and
+tests/test_gpu_shard.py (kernels)."""
 import os
 import sys
 
@@ -40,3 +42,31 @@ def test_single_rank_is_identity():
     import bench
     assert bench.allreduce_scalar(3.5, "min", "cpu", 1) == 3.5
     assert bench.aggregate_value(10, 1, 1.0) == 10 / 1e-3
+
+
+def test_sharded_workloads_keep_the_domain_and_the_state():
+    """bench.py's multi-rank workloads: same global domain as the single-GPU config, equal bricks, and every rank's
+    host input is exactly its boxes of the global seeded state."""
+    import numpy as np
+    import bench
+    from paper_1910_12578_b200 import shard, workloads as wl
+    g3, part3 = bench.sharded_config(wl.make_config(3), 8)
+    assert wl.domain(g3) == (512, 512, 512) and (g3["nbx"], g3["nby"], g3["nbz"]) == (2, 2, 2) and part3 == (2, 2, 2)
+    assert g3["dx"] == wl.make_config(3)["dx"]
+    g4, part4 = bench.sharded_config(wl.make_config(4), 4)
+    assert (g4["nbx"], g4["nby"], g4["nbz"]) == (16, 8, 4) and part4 == (2, 2, 1)
+    # small version: the single box and its 2x2x2 decomposition hold the same zones
+    one = wl.make_config(3, n=16, nspec=2)
+    g, part = bench.sharded_config(one, 2)
+    assert wl.domain(g) == wl.domain(one) and part == (2, 1, 1)
+    G1 = wl.to_global(one, wl.initial_state(one), ghosted=True)
+    full = wl.initial_state(g)
+    assert np.array_equal(wl.to_global(g, full, ghosted=True), G1)
+    for rank in range(2):
+        lc = shard.local_config(g, part)
+        pc = shard.rank_coords(part, rank)
+        lat = (lc["nbx"], lc["nby"], lc["nbz"])
+        U = np.zeros(wl.u_shape(lc))
+        bench.fill_host_state(g, U, threads=2, brick=(tuple(pc[d] * lat[d] for d in range(3)), lat))
+        ref = np.nan_to_num(full[shard.local_boxes(g, part, rank)], nan=0.0)
+        assert np.array_equal(U, ref)
