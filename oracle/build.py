@@ -1,21 +1,22 @@
-"""Build oracle/liborc.so from oracle/orc.c (plain C, -O2, no FMA contraction).
+"""Build oracle/liborc.so from oracle/*.c (plain C, -O2, no FMA contraction).
 
 Test infrastructure only.  Usage: python -m oracle.build   (or build() from Python).
 """
+import glob
 import os
 import subprocess
 
 HERE = os.path.dirname(os.path.abspath(__file__))
-SRC = os.path.join(HERE, "orc.c")
+SRC = sorted(glob.glob(os.path.join(HERE, "*.c")))
 LIB = os.path.join(HERE, "liborc.so")
 
 
 def build(force: bool = False) -> str:
     if (not force and os.path.exists(LIB)
-            and os.path.getmtime(LIB) >= os.path.getmtime(SRC)):
+            and all(os.path.getmtime(LIB) >= os.path.getmtime(f) for f in SRC)):
         return LIB
     cmd = ["gcc", "-O2", "-ffp-contract=off", "-fopenmp", "-fPIC", "-shared", "-std=c11",
-           "-Wall", "-Wextra", "-o", LIB, SRC, "-lm"]
+           "-Wall", "-Wextra", "-o", LIB] + SRC + ["-lm"]
     subprocess.run(cmd, check=True)
     return LIB
 

@@ -20,6 +20,16 @@ class OrcParams(C.Structure):
                 ("small_dens", C.c_double), ("small_pres", C.c_double)]
 
 
+MAX_REACT = 15
+
+
+class OrcReact(C.Structure):
+    """orc_react of oracle/orc_react.c: the synthetic stiff network (readings R1-R4)."""
+    _fields_ = [("cv", C.c_double), ("T0", C.c_double), ("nu", C.c_double),
+                ("rate", C.c_double * MAX_REACT), ("q", C.c_double * MAX_REACT),
+                ("max_iter", C.c_int), ("tol", C.c_double)]
+
+
 _lib = None
 _dp = C.POINTER(C.c_double)
 
@@ -47,6 +57,13 @@ def lib():
         _lib.orc_exact_riemann_star.argtypes = [C.c_double] * 7 + [_dp]
         _lib.orc_exact_riemann_sample.argtypes = [C.c_double] * 7 + [C.c_int, _dp, _dp, _dp, _dp]
         _lib.orc_num_threads.restype = C.c_int
+        R = C.POINTER(OrcReact)
+        _lib.orc_react_zone.argtypes = [R, C.c_int, C.c_double, C.c_double, _dp, _dp, _dp]
+        _lib.orc_react_zone.restype = None
+        _lib.orc_react_solve_zone.argtypes = [R, C.c_int, C.c_double, C.c_double, C.c_double, _dp, _dp]
+        _lib.orc_react_R.argtypes = [P, R, _dp, _dp]
+        _lib.orc_sdc_update_react.argtypes = [P, R, _dp, _dp, C.c_double, _dp, _dp, _dp, C.c_int, C.POINTER(_dp),
+                                              C.POINTER(_dp), _dp, _dp, C.POINTER(C.c_int)]
     return _lib
 
 
@@ -225,3 +242,82 @@ def sdc_step_nodes(cfg, U, dt, M=3, K=4, A_fn=None):
             A_new.append(None if last else A_of(Un))
         U_old, A_old = U_new, A_new
     return U_old[M - 1]
+
+
+# ---- reactions: Eq. (2) with R != 0 (oracle/orc_react.c) -------------------------
+def make_react(react: dict) -> OrcReact:
+    """react: dict(cv, T0, nu, rate=[...], q=[...], max_iter, tol) (paper_1910_12578_b200.workloads.react_params)."""
+    r = OrcReact()
+    r.cv, r.T0, r.nu = float(react["cv"]), float(react["T0"]), float(react["nu"])
+    for k, v in enumerate(react["rate"]):
+        r.rate[k] = float(v)
+    for k, v in enumerate(react["q"]):
+        r.q[k] = float(v)
+    r.max_iter, r.tol = int(react["max_iter"]), float(react["tol"])
+    return r
+
+
+def react_zone(react, rho, ke, y, jac=False):
+    """R (and dR/dy) of one zone; y = (rho X_0 .., rho E)."""
+    y = np.ascontiguousarray(y, dtype=np.float64)
+    n = len(y)
+    R = np.empty(n)
+    J = np.empty((n, n)) if jac else None
+    lib().orc_react_zone(C.byref(make_react(react)), n - 1, float(rho), float(ke), _ptr(y), _ptr(R),
+                         _ptr(J) if jac else None)
+    return (R, J) if jac else R
+
+
+def react_solve_zone(react, rho, ke, dt, c):
+    c = np.ascontiguousarray(c, dtype=np.float64)
+    y = np.empty_like(c)
+    it = lib().orc_react_solve_zone(C.byref(make_react(react)), len(c) - 1, float(rho), float(ke), float(dt), _ptr(c), _ptr(y))
+    return y, it
+
+
+def react_R(cfg, react, U, R=None):
+    if R is None:
+        R = np.empty(a_shape(cfg), dtype=np.float64)
+    _chk(lib().orc_react_R(C.byref(make_params(cfg)), C.byref(make_react(react)), _ptr(U), _ptr(R)), "react_R")
+    return R
+
+
+def sdc_update_react(cfg, react, U_next, U_m, dt_m, A_new_m, A_old_m, R_old_next, A_quad, R_quad, w_quad, R_new=None,
+                     iters=None):
+    n = len(A_quad)
+    assert n == len(R_quad) == len(w_quad)
+    aq = (_dp * max(n, 1))(*[_ptr(a) for a in A_quad])
+    rq = (_dp * max(n, 1))(*[_ptr(a) for a in R_quad])
+    w = np.ascontiguousarray(np.asarray(w_quad, dtype=np.float64))
+    if R_new is None:
+        R_new = np.empty(a_shape(cfg), dtype=np.float64)
+    ip = iters.ctypes.data_as(C.POINTER(C.c_int)) if iters is not None else None
+    _chk(lib().orc_sdc_update_react(C.byref(make_params(cfg)), C.byref(make_react(react)), _ptr(U_next), _ptr(U_m),
+                                    float(dt_m), _ptr(A_new_m), _ptr(A_old_m), _ptr(R_old_next), n, aq, rq,
+                                    _ptr(w) if n else None, _ptr(R_new), ip), "sdc_update_react")
+    return U_next, R_new
+
+
+def sdc_step_nodes_react(cfg, react, U, dt, M=3, K=4, A_fn=None):
+    """One SDC step of Eq. (2) with R != 0: M Gauss-Lobatto nodes, K iterations, every node
+    starting from U^n; the node update is implicit in R (oracle sdc_update_react), A is explicit."""
+    c, wt = lobatto_nodes_weights(M)
+    A_of = A_fn if A_fn is not None else (lambda V: advance_A(cfg, V))
+    U0 = fill_ghosts(cfg, U.copy())
+    A0, R0 = A_of(U0), react_R(cfg, react, U0)
+    A_old, R_old = [A0] * M, [R0] * M
+    U_new = [U0]
+    for k in range(K):
+        U_new, A_new, R_new = [U0], [A0], [R0]
+        for m in range(M - 1):
+            dtm = (c[m + 1] - c[m]) * dt
+            Un = U_new[m].copy()
+            _, Rn = sdc_update_react(cfg, react, Un, U_new[m], dtm, A_new[m], A_old[m], R_old[m + 1], A_old, R_old,
+                                     list(wt[m] * dt))
+            fill_ghosts(cfg, Un)
+            U_new.append(Un)
+            R_new.append(Rn)
+            last = (k == K - 1) and (m == M - 2)
+            A_new.append(None if last else A_of(Un))
+        A_old, R_old = A_new, R_new
+    return U_new[M - 1]

@@ -209,3 +209,15 @@ def random_state(cfg, seed, amp=0.3):
         E = rng.standard_exponential((cfg["nspec"], Dz, Dy, Dx))
         W[5:] = E / E.sum(axis=0, keepdims=True)
     return from_global(cfg, cons_from_prim(cfg, W))
+
+
+def react_params(nspec, stiff=1.0, nu=4.0, seed=0):
+    """Parameters of the synthetic stiff reaction chain X_0 -> X_1 -> ... (readings R1-R4; stands in for
+    the paper's 13-isotope network, whose rate tables are not available).  Input data only: rate[k] of species k ->
+    k+1 at T = T0 (spread over two decades, seeded), the specific energy release q[k], the constant c_v of the
+    temperature T = e / c_v, the exponent nu of the rates' power law, and the Newton controls."""
+    rng = np.random.default_rng([SEED, 77, int(seed), int(nspec)])
+    rate = stiff * 10.0 ** rng.uniform(0.0, 2.0, size=nspec)
+    q = 0.02 * rng.uniform(0.5, 1.5, size=nspec)
+    return dict(cv=1.5, T0=1.0, nu=float(nu), rate=[float(x) for x in rate], q=[float(x) for x in q],
+                max_iter=50, tol=1e-13)
