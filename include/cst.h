@@ -126,6 +126,38 @@ int cst_sdc_update(cst_ctx* ctx, double* U_next, const double* U_m, double dt_m,
                    const double* A_new_m, const double* A_old_m,
                    int nquad, const double* const* A_quad, const double* w_quad, void* stream);
 
+/* Reactions: Eq. (1)-(2) with R != 0 ("implicit reaction updates").
+ * The paper's 13-isotope network needs rate tables that are not available; R is a synthetic stiff chain with the same
+ * structure (readings R1-R4): species k -> k+1 at the rate lambda_k(T) = rate[k] (T/T0)^nu (the last species
+ * is stable), T = e / cv with e = E/rho - |v|^2/2, R(rho X_k) = rho (lambda_{k-1} X_{k-1} - lambda_k X_k),
+ * R(rho E) = rho sum_k q[k] lambda_k X_k, R(rho) = R(rho v) = 0.  All nspec species of the context take part
+ * (1 <= nspec <= CST_MAX_REACT, else CST_EINVAL).
+ *   cst_react_R           R <- R(U) on interior zones; R has the layout of A (components 0..3 are written as zero).
+ *   cst_sdc_update_react  the node update of Eq. (2), implicit in R: on every interior zone
+ *                           c = U_m + dt_m (A_new_m - A_old_m) - dt_m R_old_next + sum_q w_quad[q] (A_quad[q] + R_quad[q])
+ *                           U_next = c + dt_m R(U_next)
+ *                         by Newton's method per zone (first iterate c; stops when the last correction is <= tol
+ *                         relative to rho (species) / |rho E| (energy), at most max_iter iterations), and
+ *                         R_new_out <- R(U_next).  R_old_next = R^{m+1,(k)}.  A_quad, R_quad: HOST arrays of nquad
+ *                         DEVICE pointers (0 <= nquad <= CST_MAX_QUAD).  U_next may alias U_m; R_new_out may alias
+ *                         R_old_next.  Ghosts of U_next are left untouched.
+ *   cst_react_failures    *n_host (HOST) <- zones that did not converge since the last call; synchronises the stream. */
+#define CST_MAX_REACT 15
+typedef struct {
+    double cv, T0, nu;             /* T = e / cv; rates scale as (T / T0)^nu                                   */
+    double rate[CST_MAX_REACT];    /* rate[k] of species k -> k+1 at T = T0 (entry nspec-1 is ignored)         */
+    double q[CST_MAX_REACT];       /* specific energy released by the reaction of species k                    */
+    int    max_iter;               /* Newton iterations per zone (>= 1)                                        */
+    double tol;                    /* relative size of the last correction at which the iteration stops (> 0)  */
+} cst_react_params;
+int cst_set_reactions(cst_ctx* ctx, const cst_react_params* react);
+int cst_react_R(cst_ctx* ctx, const double* U, double* R, void* stream);
+int cst_sdc_update_react(cst_ctx* ctx, double* U_next, const double* U_m, double dt_m,
+                         const double* A_new_m, const double* A_old_m, const double* R_old_next,
+                         int nquad, const double* const* A_quad, const double* const* R_quad, const double* w_quad,
+                         double* R_new_out, void* stream);
+int cst_react_failures(cst_ctx* ctx, long long* n_host, void* stream);
+
 /* Fused S1-S5: A_new_m <- <A(U_m)> and the node update above with that A_new_m, in one pass over
  * U_m.  A_old_m or any A_quad[q] may be the A_new_m buffer itself (then they mean the value just
  * computed, as in the first SDC iteration where every node carries A(U^n)).  Neither output may be an

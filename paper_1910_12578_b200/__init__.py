@@ -9,4 +9,4 @@ hand-written CUDA kernels for sm_100a behind the C ABI in include/cst.h.
 """
 from . import workloads  # noqa: F401
 from .binding import Context, CstError, load  # noqa: F401
-from .drivers import sdc_step_2nd, sdc_step_nodes  # noqa: F401
+from .drivers import sdc_step_2nd, sdc_step_nodes, sdc_step_nodes_react  # noqa: F401

@@ -15,6 +15,7 @@ EXPORTS = ["cst_create", "cst_destroy", "cst_workspace_bytes", "cst_set_workspac
            "cst_advance_A_update", "cst_cfl_dt_device", "cst_cfl_dt", "cst_validate", "cst_step_host",
            "cst_set_timing", "cst_last_advance_ms", "cst_launch_count", "cst_strerror", "cst_version",
            "cst_debug_rcp_sqrt", "cst_debug_tile_count", "cst_debug_tile_map",
+           "cst_set_reactions", "cst_react_R", "cst_sdc_update_react", "cst_react_failures",
            "cst_exchange_plan", "cst_set_sublattice", "cst_exchange_info", "cst_exchange_pack", "cst_exchange_unpack"]
 
 
@@ -25,6 +26,16 @@ class CstParams(C.Structure):
                 ("gamma", C.c_double), ("grav", C.c_double * 3),
                 ("bc_lo", C.c_int * 3), ("bc_hi", C.c_int * 3),
                 ("small_dens", C.c_double), ("small_pres", C.c_double)]
+
+
+MAX_REACT = 15
+
+
+class CstReactParams(C.Structure):
+    """cst_react_params of include/cst.h: the synthetic stiff reaction chain."""
+    _fields_ = [("cv", C.c_double), ("T0", C.c_double), ("nu", C.c_double),
+                ("rate", C.c_double * MAX_REACT), ("q", C.c_double * MAX_REACT),
+                ("max_iter", C.c_int), ("tol", C.c_double)]
 
 
 class CstXseg(C.Structure):
@@ -74,6 +85,11 @@ def load():
     lib.cst_debug_tile_map.argtypes = [_vp, _vp, _vp]
     lib.cst_launch_count.argtypes = [_vp]
     lib.cst_launch_count.restype = C.c_longlong
+    lib.cst_set_reactions.argtypes = [_vp, C.POINTER(CstReactParams)]
+    lib.cst_react_R.argtypes = [_vp, _vp, _vp, _vp]
+    lib.cst_sdc_update_react.argtypes = [_vp, _vp, _vp, C.c_double, _vp, _vp, _vp, C.c_int, C.POINTER(_vp),
+                                         C.POINTER(_vp), _dp, _vp, _vp]
+    lib.cst_react_failures.argtypes = [_vp, C.POINTER(C.c_longlong), _vp]
     I3, LLP = C.POINTER(C.c_int), C.POINTER(C.c_longlong)
     lib.cst_exchange_plan.argtypes = [P, I3, C.c_int, C.c_int, C.POINTER(CstXseg), C.c_longlong]
     lib.cst_exchange_plan.restype = C.c_longlong
@@ -217,6 +233,34 @@ class Context:
         self._check(self.lib.cst_step_host(self._h, _ptr(U_host), _ptr(A_host), _ptr(U_next_host), _ptr(U_dev),
                                            _ptr(U_next_dev), _ptr(A_dev), float(dt_m), _stream(stream)),
                     "cst_step_host")
+
+    def set_reactions(self, react):
+        """react: dict(cv, T0, nu, rate=[...], q=[...], max_iter, tol) (workloads.react_params)."""
+        r = CstReactParams()
+        r.cv, r.T0, r.nu = float(react["cv"]), float(react["T0"]), float(react["nu"])
+        for k, v in enumerate(react["rate"]):
+            r.rate[k] = float(v)
+        for k, v in enumerate(react["q"]):
+            r.q[k] = float(v)
+        r.max_iter, r.tol = int(react["max_iter"]), float(react["tol"])
+        self._check(self.lib.cst_set_reactions(self._h, C.byref(r)), "cst_set_reactions")
+
+    def react_R(self, U, R, stream=None):
+        self._check(self.lib.cst_react_R(self._h, _ptr(U), _ptr(R), _stream(stream)), "cst_react_R")
+
+    def sdc_update_react(self, U_next, U_m, dt_m, A_new_m, A_old_m, R_old_next, A_quad, R_quad, w_quad, R_new_out,
+                         stream=None):
+        n, arr, w = self._quad(A_quad, w_quad)
+        assert len(R_quad) == n
+        rarr = (_vp * max(n, 1))(*[_ptr(a) for a in R_quad])
+        self._check(self.lib.cst_sdc_update_react(self._h, _ptr(U_next), _ptr(U_m), float(dt_m), _ptr(A_new_m),
+                                                  _ptr(A_old_m), _ptr(R_old_next), n, arr, rarr, w, _ptr(R_new_out),
+                                                  _stream(stream)), "cst_sdc_update_react")
+
+    def react_failures(self, stream=None):
+        n = C.c_longlong(0)
+        self._check(self.lib.cst_react_failures(self._h, C.byref(n), _stream(stream)), "cst_react_failures")
+        return n.value
 
     def set_sublattice(self, global_nb, part, rank):
         g = (C.c_int * 3)(*[int(x) for x in global_nb])

@@ -64,6 +64,7 @@ extern "C" int cst_create(const cst_params* p, cst_ctx** out)
     c->ws = nullptr; c->ws_bytes = 0;
     c->timing = 0;
     c->xplan = nullptr;
+    c->has_react = 0;
     for (int n = 0; n < 3; ++n) c->ev[n] = nullptr;
     int dev = 0;
     cudaError_t e = cudaGetDevice(&dev);
@@ -209,6 +210,53 @@ extern "C" int cst_step_host(cst_ctx* c, const double* U_host, double* A_host, d
     if (e == cudaSuccess) e = cudaMemcpyAsync(U_next_host, U_next_dev, ub, cudaMemcpyDeviceToHost, st);
     if (e == cudaSuccess) e = cudaStreamSynchronize(st);
     return e == cudaSuccess ? CST_OK : cuda_fail(e);
+}
+
+extern "C" int cst_set_reactions(cst_ctx* c, const cst_react_params* r)
+{
+    if (!c || !r) return CST_EINVAL;
+    if (c->g.nspec < 1 || c->g.nspec > CST_MAX_REACT) return CST_EINVAL;
+    if (!(r->cv > 0) || !(r->T0 > 0) || r->max_iter < 1 || !(r->tol > 0)) return CST_EINVAL;
+    const unsigned long long zero = 0;
+    cudaError_t e = cudaMemcpyAsync(c->d_scratch + 3, &zero, sizeof(zero), cudaMemcpyHostToDevice, 0);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(0);
+    if (e != cudaSuccess) return cuda_fail(e);
+    c->react = *r;
+    c->has_react = 1;
+    return CST_OK;
+}
+
+extern "C" int cst_react_R(cst_ctx* c, const double* U, double* R, void* stream)
+{
+    if (!c || !U || !R) return CST_EINVAL;
+    return check_launch(launch_react_R(c, U, R, (cudaStream_t)stream));
+}
+
+extern "C" int cst_sdc_update_react(cst_ctx* c, double* U_next, const double* U_m, double dt_m,
+                                    const double* A_new_m, const double* A_old_m, const double* R_old_next,
+                                    int nquad, const double* const* A_quad, const double* const* R_quad,
+                                    const double* w_quad, double* R_new_out, void* stream)
+{
+    if (!c || !U_next || !U_m || !A_new_m || !A_old_m || !R_old_next || !R_new_out) return CST_EINVAL;
+    if (nquad < 0 || nquad > CST_MAX_QUAD || (nquad > 0 && (!A_quad || !R_quad || !w_quad))) return CST_EINVAL;
+    for (int n = 0; n < nquad; ++n) if (!A_quad[n] || !R_quad[n]) return CST_EINVAL;
+    return check_launch(launch_sdc_update_react(c, U_next, U_m, dt_m, A_new_m, A_old_m, R_old_next, nquad, A_quad,
+                                                R_quad, w_quad, R_new_out, (cudaStream_t)stream));
+}
+
+extern "C" int cst_react_failures(cst_ctx* c, long long* n_host, void* stream)
+{
+    if (!c || !n_host || !c->has_react) return CST_EINVAL;
+    cudaStream_t st = (cudaStream_t)stream;
+    unsigned long long n = 0;
+    const unsigned long long zero = 0;
+    cudaError_t e = cudaMemcpyAsync(&n, c->d_scratch + 3, sizeof(n), cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(c->d_scratch + 3, &zero, sizeof(zero), cudaMemcpyHostToDevice, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    if (e != cudaSuccess) return cuda_fail(e);
+    *n_host = (long long)n;
+    return CST_OK;
 }
 
 extern "C" int cst_set_sublattice(cst_ctx* c, const int global_nb[3], const int part[3], int rank)

@@ -38,6 +38,8 @@ struct cst_ctx {
     int timing;              // cst_set_timing: record events around the kernels of the advance calls
     cudaEvent_t ev[3];       // before hydro, between hydro and species, after species
     struct XPlan* xplan;     // cst_set_sublattice: ghost-exchange plan with the neighbouring ranks (exchange.cu)
+    cst_react_params react;  // cst_set_reactions (react.cu)
+    int has_react;
 };
 
 struct UpdArgs;
@@ -67,6 +69,11 @@ int launch_sdc_update(cst_ctx*, double* U_next, const double* U_m, double dt_m,
                       const double* A_new_m, const double* A_old_m, const QuadArgs& q, cudaStream_t);
 int launch_cfl(cst_ctx*, const double* U, double cfl, double* dt_out_dev, cudaStream_t);
 int launch_validate(cst_ctx*, const double* U, cudaStream_t);   // count left in d_scratch[2]
+// react.cu: R != 0
+int launch_react_R(cst_ctx*, const double* U, double* R, cudaStream_t);
+int launch_sdc_update_react(cst_ctx*, double* U_next, const double* U_m, double dt_m, const double* A_new_m,
+                            const double* A_old_m, const double* R_old_next, int nquad, const double* const* A_quad,
+                            const double* const* R_quad, const double* w_quad, double* R_new, cudaStream_t);
 // exchange.cu: box lattice sharded over ranks
 int xplan_create(cst_ctx*, const int global_nb[3], const int part[3], int rank);
 void xplan_destroy(cst_ctx*);

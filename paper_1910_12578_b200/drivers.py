@@ -54,3 +54,37 @@ def sdc_step_nodes(ctx, U, dt, M=3, K=4, stream=None):
         A_old = A_new
     if M > 1:
         U.copy_(U_nodes[M - 1])
+
+
+def sdc_step_nodes_react(ctx, U, dt, M=3, K=4, stream=None):
+    """One SDC step of Eq. (2) with R != 0: M Gauss-Lobatto nodes, K iterations, A explicit,
+    R implicit (cst_sdc_update_react; needs ctx.set_reactions).  Library calls only.  U: state with interior valid;
+    result left in U (interior)."""
+    import torch
+    wt = _SDC_WEIGHTS[M]
+    dtm = dt / (M - 1)
+    ashape = (U.shape[0], U.shape[1], U.shape[2] - 8, U.shape[3] - 8, U.shape[4] - 8)
+    new_A = lambda: torch.empty(ashape, dtype=U.dtype, device=U.device)
+    ctx.fill_ghosts(U, stream)
+    A0, R0 = new_A(), new_A()
+    ctx.advance_A(U, A0, stream)
+    ctx.react_R(U, R0, stream)
+    A_old, R_old = [A0] * M, [R0] * M
+    A_buf = [[new_A() for _ in range(M - 1)] for _ in range(2)]
+    R_buf = [[new_A() for _ in range(M - 1)] for _ in range(2)]
+    U_nodes = [U] + [torch.empty_like(U) for _ in range(M - 1)]
+    for k in range(K):
+        A_new, R_new = [A0], [R0]
+        for m in range(M - 1):
+            Rn = R_buf[k % 2][m]
+            ctx.sdc_update_react(U_nodes[m + 1], U_nodes[m], dtm, A_new[m], A_old[m], R_old[m + 1], A_old, R_old,
+                                 [w * dt for w in wt[m]], Rn, stream)
+            R_new.append(Rn)
+            if k == K - 1 and m == M - 2:
+                break
+            ctx.fill_ghosts(U_nodes[m + 1], stream)
+            ctx.advance_A(U_nodes[m + 1], A_buf[k % 2][m], stream)
+            A_new.append(A_buf[k % 2][m])
+        A_old, R_old = A_new, R_new
+    if M > 1:
+        U.copy_(U_nodes[M - 1])
