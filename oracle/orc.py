@@ -57,6 +57,7 @@ def lib():
         _lib.orc_exact_riemann_star.argtypes = [C.c_double] * 7 + [_dp]
         _lib.orc_exact_riemann_sample.argtypes = [C.c_double] * 7 + [C.c_int, _dp, _dp, _dp, _dp]
         _lib.orc_num_threads.restype = C.c_int
+        _lib.orc_diffusion.argtypes = [P, C.c_double, C.c_double, _dp, _dp]
         R = C.POINTER(OrcReact)
         _lib.orc_react_zone.argtypes = [R, C.c_int, C.c_double, C.c_double, _dp, _dp, _dp]
         _lib.orc_react_zone.restype = None
@@ -321,3 +322,19 @@ def sdc_step_nodes_react(cfg, react, U, dt, M=3, K=4, A_fn=None):
             A_new.append(None if last else A_of(Un))
         A_old, R_old = A_new, R_new
     return U_new[M - 1]
+
+
+# ---- explicit thermal diffusion as an extra term of A (oracle/orc_diffuse.c) --------
+def diffusion(cfg, kth, cv, U):
+    """D[b][k][j][i] = k_th lap T on interior zones (ghosts of U filled)."""
+    sh = a_shape(cfg)
+    D = np.empty((sh[0],) + sh[2:], dtype=np.float64)
+    _chk(lib().orc_diffusion(C.byref(make_params(cfg)), float(kth), float(cv), _ptr(U), _ptr(D)), "diffusion")
+    return D
+
+
+def advance_A_diffuse(cfg, kth, cv, U):
+    """<A(U)> with the diffusion term added to the energy component."""
+    A = advance_A(cfg, U)
+    A[:, 4] += diffusion(cfg, kth, cv, U)
+    return A
