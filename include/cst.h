@@ -126,6 +126,14 @@ int cst_sdc_update(cst_ctx* ctx, double* U_next, const double* U_m, double dt_m,
                    const double* A_new_m, const double* A_old_m,
                    int nquad, const double* const* A_quad, const double* w_quad, void* stream);
 
+/* Explicit thermal diffusion as an extra term of A ("thermal diffusion", "explicit diffusion"; SURVEY 8(f)
+ * NEXT-4; readings D1-D3).  With kth > 0 every later cst_advance_A / cst_advance_A_update / cst_step_host adds
+ *   k_th lap T,  T = p / ((gamma - 1) rho cv),  p the floored gamma-law pressure of S1,
+ * (second-order centred differences on the +-1 star, summed ((x + y) + z)) to the rho E component of A, the fused
+ * node update included.  Constant conductivity and c_v: the paper's conductivity tables are not available.
+ * kth = 0 switches the term off (default).  CST_EINVAL: kth < 0 or cv <= 0. */
+int cst_set_diffusion(cst_ctx* ctx, double kth, double cv);
+
 /* Reactions: Eq. (1)-(2) with R != 0 ("implicit reaction updates").
  * The paper's 13-isotope network needs rate tables that are not available; R is a synthetic stiff chain with the same
  * structure (readings R1-R4): species k -> k+1 at the rate lambda_k(T) = rate[k] (T/T0)^nu (the last species

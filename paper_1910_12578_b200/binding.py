@@ -15,7 +15,7 @@ EXPORTS = ["cst_create", "cst_destroy", "cst_workspace_bytes", "cst_set_workspac
            "cst_advance_A_update", "cst_cfl_dt_device", "cst_cfl_dt", "cst_validate", "cst_step_host",
            "cst_set_timing", "cst_last_advance_ms", "cst_launch_count", "cst_strerror", "cst_version",
            "cst_debug_rcp_sqrt", "cst_debug_tile_count", "cst_debug_tile_map",
-           "cst_set_reactions", "cst_react_R", "cst_sdc_update_react", "cst_react_failures",
+           "cst_set_diffusion", "cst_set_reactions", "cst_react_R", "cst_sdc_update_react", "cst_react_failures",
            "cst_exchange_plan", "cst_set_sublattice", "cst_exchange_info", "cst_exchange_pack", "cst_exchange_unpack"]
 
 
@@ -85,6 +85,7 @@ def load():
     lib.cst_debug_tile_map.argtypes = [_vp, _vp, _vp]
     lib.cst_launch_count.argtypes = [_vp]
     lib.cst_launch_count.restype = C.c_longlong
+    lib.cst_set_diffusion.argtypes = [_vp, C.c_double, C.c_double]
     lib.cst_set_reactions.argtypes = [_vp, C.POINTER(CstReactParams)]
     lib.cst_react_R.argtypes = [_vp, _vp, _vp, _vp]
     lib.cst_sdc_update_react.argtypes = [_vp, _vp, _vp, C.c_double, _vp, _vp, _vp, C.c_int, C.POINTER(_vp),
@@ -233,6 +234,9 @@ class Context:
         self._check(self.lib.cst_step_host(self._h, _ptr(U_host), _ptr(A_host), _ptr(U_next_host), _ptr(U_dev),
                                            _ptr(U_next_dev), _ptr(A_dev), float(dt_m), _stream(stream)),
                     "cst_step_host")
+
+    def set_diffusion(self, kth, cv):
+        self._check(self.lib.cst_set_diffusion(self._h, float(kth), float(cv)), "cst_set_diffusion")
 
     def set_reactions(self, react):
         """react: dict(cv, T0, nu, rate=[...], q=[...], max_iter, tol) (workloads.react_params)."""

@@ -44,6 +44,8 @@ int launch_advance_A(cst_ctx* ctx, const double* U, double* A, double* U_next, d
     if (ctx->timing) cudaEventRecord(ctx->ev[1], st);
     rc = launch_advect_species(ctx, U, A, up, st);
     if (ctx->timing) cudaEventRecord(ctx->ev[2], st);
+    if (!rc && ctx->diff_kth != 0.0)     // optional extra term of A (cst_set_diffusion); the fused update is completed too
+        rc = launch_diffuse_add(ctx, U, A, (up.nr >= 0) ? U_next : nullptr, up.ca, st);
     if (rc || !split) return rc;
     // too many distinct arrays for the fused epilogue: A first, then the plain update kernel
     return launch_sdc_update(ctx, U_next, U, dt_m, A, A_old_m, q, st);

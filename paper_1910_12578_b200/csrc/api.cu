@@ -65,6 +65,7 @@ extern "C" int cst_create(const cst_params* p, cst_ctx** out)
     c->timing = 0;
     c->xplan = nullptr;
     c->has_react = 0;
+    c->diff_kth = 0.0; c->diff_cv = 1.0;
     for (int n = 0; n < 3; ++n) c->ev[n] = nullptr;
     int dev = 0;
     cudaError_t e = cudaGetDevice(&dev);
@@ -210,6 +211,13 @@ extern "C" int cst_step_host(cst_ctx* c, const double* U_host, double* A_host, d
     if (e == cudaSuccess) e = cudaMemcpyAsync(U_next_host, U_next_dev, ub, cudaMemcpyDeviceToHost, st);
     if (e == cudaSuccess) e = cudaStreamSynchronize(st);
     return e == cudaSuccess ? CST_OK : cuda_fail(e);
+}
+
+extern "C" int cst_set_diffusion(cst_ctx* c, double kth, double cv)
+{
+    if (!c || !(kth >= 0.0) || !(cv > 0.0)) return CST_EINVAL;
+    c->diff_kth = kth; c->diff_cv = cv;
+    return CST_OK;
 }
 
 extern "C" int cst_set_reactions(cst_ctx* c, const cst_react_params* r)
