@@ -192,6 +192,45 @@ void orc_ppm_line(int n, const double *q, double *qm, double *qp)
     free(dq); free(ed);
 }
 
+/* --------------------------------------------------- S2b (optional) --- */
+/* Shock flattening (CW84 appendix; "[15, 16]").  OFF on the graded
+ * path (orc_advance_A); orc_advance_A_flat switches it on.  Readings F1-F4:
+ *  F1  along direction d, with u the velocity component along d:
+ *        dp = p_{i+1} - p_{i-1},  dp2 = p_{i+2} - p_{i-2},  z = |dp| / max(|dp2|, small_pres),
+ *        chi~_i = clamp(1 - (z - 0.75) / (0.85 - 0.75), 0, 1)   if the zone sits in a shock, i.e.
+ *        u_{i-1} - u_{i+1} >= 0 (compression) and |dp| / min(p_{i+1}, p_{i-1}) > 1/3;  else chi~_i = 1;
+ *  F2  chi^d_i = min(chi~_i, chi~_{i+s}),  s = -1 if dp > 0 else +1  (the neighbour on the low-pressure side);
+ *  F3  chi_i = min over the three directions of chi^d_i;
+ *  F4  every parabola of the zone, in every direction and for every variable:  q+- <- chi q+- + (1 - chi) q.
+ * orc_flatten_tilde: chi~ for zones i = 2..n-3 of one line (others untouched);
+ * orc_flatten_line : chi^d for zones i = 3..n-4 of one line. */
+void orc_flatten_tilde(int n, const double *p, const double *u, double small_pres, double *ct)
+{
+    for (int i = 2; i <= n - 3; ++i) {
+        const double dp = p[i + 1] - p[i - 1], dp2 = p[i + 2] - p[i - 2];
+        const double den = fabs(dp2) > small_pres ? fabs(dp2) : small_pres;
+        const double z = fabs(dp) / den;
+        double zeta = 1.0 - (z - 0.75) / (0.85 - 0.75);
+        if (zeta < 0.0) zeta = 0.0;
+        if (zeta > 1.0) zeta = 1.0;
+        const double pmin = p[i + 1] < p[i - 1] ? p[i + 1] : p[i - 1];
+        const int shock = (u[i - 1] - u[i + 1] >= 0.0) && (fabs(dp) / pmin > 1.0 / 3.0);
+        ct[i] = shock ? zeta : 1.0;
+    }
+}
+
+void orc_flatten_line(int n, const double *p, const double *u, double small_pres, double *chi)
+{
+    double *ct = (double *)malloc(sizeof(double) * (size_t)n);
+    orc_flatten_tilde(n, p, u, small_pres, ct);
+    for (int i = 3; i <= n - 4; ++i) {
+        const double dp = p[i + 1] - p[i - 1];
+        const double nb = dp > 0.0 ? ct[i - 1] : ct[i + 1];
+        chi[i] = ct[i] < nb ? ct[i] : nb;
+    }
+    free(ct);
+}
+
 /* ------------------------------------------------------------------ S3 --- */
 /* HLLC flux through a face whose normal is direction d (0,1,2)
  * (BASELINE north_star names HLLC; construction: Toro ch. 10; pressure-based
@@ -275,12 +314,19 @@ void orc_hllc(int N, int d, double gamma, const double *WL, const double *WR, do
  *      summed ((x+y)+z) (Q13);  S[rho v_d] = rho g_d,
  *      S[rho E] = sum_d (rho v_d) g_d from the zone-centre U (Q14). */
 static void line_fluxes(const orc_params *p, int d, int n, const double *Wline /* [N][n+2ng] */,
-                        double *Fline /* [N][n+1] */, double *scr)
+                        double *Fline /* [N][n+1] */, double *scr, const double *chiline /* [n+2ng] or NULL */)
 {
     const int ng = p->ng, N = 5 + p->nspec, e = n + 2 * ng;
     double *qm = scr, *qp = scr + (size_t)N * e;
     for (int c = 0; c < N; ++c)
         orc_ppm_line(e, Wline + (size_t)c * e, qm + (size_t)c * e, qp + (size_t)c * e);
+    if (chiline)                                     /* F4: zones -1 .. n carry the parabolas the faces use */
+        for (int c = 0; c < N; ++c)
+        for (int i = ng - 1; i <= n + ng; ++i) {
+            const double x = chiline[i], q = Wline[(size_t)c * e + i];
+            qm[(size_t)c * e + i] = x * qm[(size_t)c * e + i] + (1.0 - x) * q;
+            qp[(size_t)c * e + i] = x * qp[(size_t)c * e + i] + (1.0 - x) * q;
+        }
     double WL[64], WR[64], F[64];
     for (int f = 0; f <= n; ++f) {
         const int zl = f - 1 + ng, zr = f + ng;   /* ghosted indices of the two zones */
@@ -294,7 +340,7 @@ static void line_fluxes(const orc_params *p, int d, int n, const double *Wline /
     }
 }
 
-int orc_advance_A(const orc_params *p, const double *U, double *A)
+static int advance_A_impl(const orc_params *p, const double *U, double *A, int flatten)
 {
     int rc = check_params(p);
     if (rc) return rc;
@@ -309,7 +355,8 @@ int orc_advance_A(const orc_params *p, const double *U, double *A)
     double *Fx = (double *)malloc(sizeof(double) * (size_t)N * (nx + 1) * ny * nz);
     double *Fy = (double *)malloc(sizeof(double) * (size_t)N * nx * (ny + 1) * nz);
     double *Fz = (double *)malloc(sizeof(double) * (size_t)N * nx * ny * (nz + 1));
-    if (!W || !Fx || !Fy || !Fz) { free(W); free(Fx); free(Fy); free(Fz); return ORC_ENOMEM; }
+    double *chi = flatten ? (double *)malloc(sizeof(double) * (size_t)nzone_g) : NULL;
+    if (!W || !Fx || !Fy || !Fz || (flatten && !chi)) { free(W); free(Fx); free(Fy); free(Fz); free(chi); return ORC_ENOMEM; }
     long emax = ex > ey ? ex : ey; if (ez > emax) emax = ez;
 
     for (long b = 0; b < nbox; ++b) {
@@ -327,10 +374,31 @@ int orc_advance_A(const orc_params *p, const double *U, double *A)
                 for (int c = 0; c < N; ++c) W[c * nzone_g + z] = Wz[c];
             }
         }
+        /* (1b) optional flattening coefficient on zones -1 .. n of every direction (F1-F3); needs the whole shell */
+        if (flatten) {
+            for (long z = 0; z < nzone_g; ++z) chi[z] = 1.0;
+            double *pl = (double *)malloc(sizeof(double) * (size_t)emax), *ul = (double *)malloc(sizeof(double) * (size_t)emax);
+            double *cl = (double *)malloc(sizeof(double) * (size_t)emax);
+            for (int d = 0; d < 3; ++d) {
+                const long e_d = d == 0 ? ex : d == 1 ? ey : ez, st = d == 0 ? 1 : d == 1 ? ex : ex * ey;
+                const long ea = d == 0 ? ey : ex, eb = d == 2 ? ey : ez;          /* the two other extents */
+                const long sa = d == 0 ? ex : 1, sb = d == 2 ? ex : ex * ey;      /* and their strides */
+                for (long bb = ng - 1; bb <= eb - ng; ++bb)
+                for (long aa = ng - 1; aa <= ea - ng; ++aa) {
+                    const long z0 = aa * sa + bb * sb;
+                    for (long i = 0; i < e_d; ++i) { pl[i] = W[4 * nzone_g + z0 + i * st]; ul[i] = W[(1 + d) * nzone_g + z0 + i * st]; }
+                    orc_flatten_line((int)e_d, pl, ul, p->small_pres, cl);
+                    for (long i = ng - 1; i <= e_d - ng; ++i)
+                        if (cl[i] < chi[z0 + i * st]) chi[z0 + i * st] = cl[i];        /* F3 */
+                }
+            }
+            free(pl); free(ul); free(cl);
+        }
         /* (2) fluxes, direction by direction */
         #pragma omp parallel
         {
             double *Wl = (double *)malloc(sizeof(double) * (size_t)N * emax);
+            double *Cl = (double *)malloc(sizeof(double) * (size_t)emax);
             double *Fl = (double *)malloc(sizeof(double) * (size_t)N * emax);
             double *sc = (double *)malloc(sizeof(double) * (size_t)2 * N * emax);
             /* x lines */
@@ -340,7 +408,8 @@ int orc_advance_A(const orc_params *p, const double *U, double *A)
                 for (int c = 0; c < N; ++c)
                 for (long i = 0; i < ex; ++i)
                     Wl[c * ex + i] = W[c * nzone_g + ((k + ng) * ey + (j + ng)) * ex + i];
-                line_fluxes(p, 0, nx, Wl, Fl, sc);
+                if (chi) for (long i = 0; i < ex; ++i) Cl[i] = chi[((k + ng) * ey + (j + ng)) * ex + i];
+                line_fluxes(p, 0, nx, Wl, Fl, sc, chi ? Cl : NULL);
                 for (int c = 0; c < N; ++c)
                 for (long f = 0; f <= nx; ++f)
                     Fx[((c * (long)nz + k) * ny + j) * (nx + 1) + f] = Fl[c * (nx + 1) + f];
@@ -352,7 +421,8 @@ int orc_advance_A(const orc_params *p, const double *U, double *A)
                 for (int c = 0; c < N; ++c)
                 for (long j = 0; j < ey; ++j)
                     Wl[c * ey + j] = W[c * nzone_g + ((k + ng) * ey + j) * ex + (i + ng)];
-                line_fluxes(p, 1, ny, Wl, Fl, sc);
+                if (chi) for (long j = 0; j < ey; ++j) Cl[j] = chi[((k + ng) * ey + j) * ex + (i + ng)];
+                line_fluxes(p, 1, ny, Wl, Fl, sc, chi ? Cl : NULL);
                 for (int c = 0; c < N; ++c)
                 for (long f = 0; f <= ny; ++f)
                     Fy[((c * (long)nz + k) * (ny + 1) + f) * nx + i] = Fl[c * (ny + 1) + f];
@@ -364,12 +434,13 @@ int orc_advance_A(const orc_params *p, const double *U, double *A)
                 for (int c = 0; c < N; ++c)
                 for (long k = 0; k < ez; ++k)
                     Wl[c * ez + k] = W[c * nzone_g + (k * ey + (j + ng)) * ex + (i + ng)];
-                line_fluxes(p, 2, nz, Wl, Fl, sc);
+                if (chi) for (long k = 0; k < ez; ++k) Cl[k] = chi[(k * ey + (j + ng)) * ex + (i + ng)];
+                line_fluxes(p, 2, nz, Wl, Fl, sc, chi ? Cl : NULL);
                 for (int c = 0; c < N; ++c)
                 for (long f = 0; f <= nz; ++f)
                     Fz[((c * (long)(nz + 1) + f) * ny + j) * nx + i] = Fl[c * (nz + 1) + f];
             }
-            free(Wl); free(Fl); free(sc);
+            free(Wl); free(Fl); free(sc); free(Cl);
         }
         /* (3) divergence + source */
         #pragma omp parallel for schedule(static)
@@ -396,8 +467,20 @@ int orc_advance_A(const orc_params *p, const double *U, double *A)
             }
         }
     }
-    free(W); free(Fx); free(Fy); free(Fz);
+    free(W); free(Fx); free(Fy); free(Fz); free(chi);
     return ORC_OK;
+}
+
+int orc_advance_A(const orc_params *p, const double *U, double *A)
+{
+    return advance_A_impl(p, U, A, 0);
+}
+
+/* <A(U)> with CW84 shock flattening switched on (readings F1-F4 above); reads the WHOLE 4-deep shell (edges and
+ * corners included: the coefficient of a face-ghost zone looks three zones sideways). */
+int orc_advance_A_flat(const orc_params *p, const double *U, double *A)
+{
+    return advance_A_impl(p, U, A, 1);
 }
 
 /* ------------------------------------------------------------------ S5 --- */

@@ -41,6 +41,9 @@ def lib():
         P = C.POINTER(OrcParams)
         _lib.orc_fill_ghosts.argtypes = [P, _dp]
         _lib.orc_advance_A.argtypes = [P, _dp, _dp]
+        _lib.orc_advance_A_flat.argtypes = [P, _dp, _dp]
+        _lib.orc_flatten_line.argtypes = [C.c_int, _dp, _dp, C.c_double, _dp]
+        _lib.orc_flatten_line.restype = None
         _lib.orc_sdc_update.argtypes = [P, _dp, _dp, C.c_double, _dp, _dp, C.c_int,
                                         C.POINTER(_dp), _dp]
         _lib.orc_cfl_dt.argtypes = [P, _dp, C.c_double, _dp]
@@ -114,6 +117,24 @@ def advance_A(cfg, U, A=None):
         A = np.empty(a_shape(cfg), dtype=np.float64)
     _chk(lib().orc_advance_A(C.byref(make_params(cfg)), _ptr(U), _ptr(A)), "advance_A")
     return A
+
+
+def advance_A_flat(cfg, U, A=None):
+    """<A(U)> with CW84 shock flattening (readings F1-F4); the whole ghost shell of U must be filled."""
+    assert U.shape == u_shape(cfg)
+    if A is None:
+        A = np.empty(a_shape(cfg), dtype=np.float64)
+    _chk(lib().orc_advance_A_flat(C.byref(make_params(cfg)), _ptr(U), _ptr(A)), "advance_A_flat")
+    return A
+
+
+def flatten_line(p, u, small_pres=1e-200):
+    """chi^d of one line (F1-F2); valid for zones 3..n-4, 1 elsewhere."""
+    p = np.ascontiguousarray(p, dtype=np.float64)
+    u = np.ascontiguousarray(u, dtype=np.float64)
+    chi = np.ones_like(p)
+    lib().orc_flatten_line(len(p), _ptr(p), _ptr(u), float(small_pres), _ptr(chi))
+    return chi
 
 
 def sdc_update(cfg, U_next, U_m, dt_m, A_new_m, A_old_m, A_quad, w_quad):
