@@ -126,6 +126,15 @@ int cst_sdc_update(cst_ctx* ctx, double* U_next, const double* U_m, double dt_m,
                    const double* A_new_m, const double* A_old_m,
                    int nquad, const double* const* A_quad, const double* w_quad, void* stream);
 
+/* Shock flattening (Colella & Woodward 1984, appendix; P:L52 ref [15]; DESIGN.md readings
+ * F1-F4), an option that is OFF by default (the graded path, Q4).  With on != 0 every later
+ * cst_advance_A / cst_advance_A_update / cst_step_host first computes the flattening coefficient chi of every zone
+ * (min over the three directions of CW84's pressure-jump / compression test) and blends every PPM parabola with its
+ * zone average, q+- <- chi q+- + (1 - chi) q.  It reads the WHOLE 4-deep ghost shell (edges and corners included) and
+ * runs on the general (any box shape) kernels.  Switching it on enlarges cst_workspace_bytes() by one double per
+ * ghosted zone: call it BEFORE sizing / setting the workspace (else the advance calls return CST_ENOWORKSPACE). */
+int cst_set_flattening(cst_ctx* ctx, int on);
+
 /* Explicit thermal diffusion as an extra term of A ("thermal diffusion", "explicit diffusion"; SURVEY 8(f)
  * NEXT-4; readings D1-D3).  With kth > 0 every later cst_advance_A / cst_advance_A_update / cst_step_host adds
  *   k_th lap T,  T = p / ((gamma - 1) rho cv),  p the floored gamma-law pressure of S1,

@@ -6,9 +6,10 @@
 // (tile.cuh, sweep.cuh); DESIGN.md section 6 has the design and its roofline.
 #include "tile.cuh"
 
-long long workspace_bytes(const Geom& g)
-{
-    return (ws_rinv_doubles(g) + ws_fm_doubles(g)) * (long long)sizeof(double);
+long long workspace_bytes(const cst_ctx* ctx)
+{   // [rinv][Fm] and, with flattening switched on, [chi] (one double per ghosted zone)
+    const Geom& g = ctx->g;
+    return (ws_rinv_doubles(g) + ws_fm_doubles(g) + (ctx->flatten ? ws_rinv_doubles(g) : 0)) * (long long)sizeof(double);
 }
 
 // Eq. (2) with R = 0 -> coefficient list (tile.cuh UpdArgs).  Returns false when more than
@@ -33,13 +34,15 @@ static bool make_upd(UpdArgs& up, const double* U, double* A, double* U_next, do
 int launch_advance_A(cst_ctx* ctx, const double* U, double* A, double* U_next, double dt_m,
                      const double* A_old_m, const QuadArgs& q, bool fused, cudaStream_t st)
 {
-    if (!ctx->ws || ctx->ws_bytes < workspace_bytes(ctx->g)) return CST_ENOWORKSPACE;
+    if (!ctx->ws || ctx->ws_bytes < workspace_bytes(ctx)) return CST_ENOWORKSPACE;
     UpdArgs up{};
     up.nr = -1; up.U_m = U; up.A_base = A;
     bool split = false;
     if (fused && !make_upd(up, U, A, U_next, dt_m, A_old_m, q)) { up.nr = -1; split = true; }
+    int rc = CST_OK;
+    if (ctx->flatten && (rc = launch_flatten(ctx, U, st)) != CST_OK) return rc;
     if (ctx->timing) cudaEventRecord(ctx->ev[0], st);
-    int rc = launch_advect_hydro(ctx, U, A, up, st);
+    rc = launch_advect_hydro(ctx, U, A, up, st);
     if (rc) return rc;
     if (ctx->timing) cudaEventRecord(ctx->ev[1], st);
     rc = launch_advect_species(ctx, U, A, up, st);

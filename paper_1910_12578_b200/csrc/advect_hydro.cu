@@ -214,11 +214,11 @@ __device__ __forceinline__ void hydro_sweep_full(const Geom& g, const TileCoord&
 }
 
 // --------------------------------------------------------------------------- any tile extent ----
-template <int D, int NR>
+template <int D, int NR, bool FLAT>
 __device__ __forceinline__ void hydro_sweep(const Geom& g, const TileCoord& tc, const double* __restrict__ Ub,
                                             double* __restrict__ part, double* __restrict__ fm_tile,
                                             double* __restrict__ rinv_b, double* __restrict__ A,
-                                            const UpdArgs& up)
+                                            const UpdArgs& up, const double* __restrict__ chi_b)
 {
     const int ng = CST_NG;
     const int tid = threadIdx.x, a = tid & (TILE - 1), b = tid >> 4;
@@ -275,8 +275,14 @@ __device__ __forceinline__ void hydro_sweep(const Geom& g, const TileCoord& tc, 
 #pragma unroll
             for (int c = 0; c < 5; ++c) w[c].warm3(W[c]);
         } else {
+            if (FLAT) {                                  // optional CW84 flattening of the parabola of zone p-2
+                const double x = chi_b[z0 + (long long)(p - 2) * stride];
 #pragma unroll
-            for (int c = 0; c < 5; ++c) w[c].push(W[c]);
+                for (int c = 0; c < 5; ++c) w[c].push_flat(W[c], x);
+            } else {
+#pragma unroll
+                for (int c = 0; c < 5; ++c) w[c].push(W[c]);
+            }
             if (p >= 2) {
                 // face f = p-2 between zones p-3 and p-2
                 double WL[5], WR[5], F[5];
@@ -338,17 +344,18 @@ __device__ __forceinline__ void hydro_sweep(const Geom& g, const TileCoord& tc, 
     }
 }
 
-template <int NR>
+template <int NR, bool FLAT>
 __global__ void __launch_bounds__(NTHR, 1)
 k_advect_hydro(Geom g, TileGeom tg, const double* __restrict__ U, double* __restrict__ A,
-               double* __restrict__ rinv, double* __restrict__ Fm, UpdArgs up, bool x_vec)
+               double* __restrict__ rinv, double* __restrict__ Fm, UpdArgs up, bool x_vec, const double* __restrict__ chi)
 {
     extern __shared__ double part[];                   // [5][TILE][TILE][PART_PITCH]
     const TileCoord tc = tile_coord(g, tg, blockIdx.x);
     const double* Ub = U + (long long)tc.b * g.box_g;
     double* rinv_b = rinv + (long long)tc.b * g.comp_g;
     double* fm_tile = Fm + tc.tile * 3LL * (TILE + 1) * NTHR;
-    const bool full = (tc.tx == TILE) && (tc.ty == TILE) && (tc.tz == TILE) && x_vec;
+    const double* chi_b = FLAT ? chi + (long long)tc.b * g.comp_g : nullptr;
+    const bool full = !FLAT && (tc.tx == TILE) && (tc.ty == TILE) && (tc.tz == TILE) && x_vec;   // flattening: general body only
     if (full) {
         hydro_sweep_full<0, NR>(g, tc, Ub, part, fm_tile, rinv_b, A, up);
         __syncthreads();
@@ -356,11 +363,11 @@ k_advect_hydro(Geom g, TileGeom tg, const double* __restrict__ U, double* __rest
         __syncthreads();
         hydro_sweep_full<2, NR>(g, tc, Ub, part, fm_tile, rinv_b, A, up);
     } else {
-        hydro_sweep<0, NR>(g, tc, Ub, part, fm_tile, rinv_b, A, up);
+        hydro_sweep<0, NR, FLAT>(g, tc, Ub, part, fm_tile, rinv_b, A, up, chi_b);
         __syncthreads();
-        hydro_sweep<1, NR>(g, tc, Ub, part, fm_tile, rinv_b, A, up);
+        hydro_sweep<1, NR, FLAT>(g, tc, Ub, part, fm_tile, rinv_b, A, up, chi_b);
         __syncthreads();
-        hydro_sweep<2, NR>(g, tc, Ub, part, fm_tile, rinv_b, A, up);
+        hydro_sweep<2, NR, FLAT>(g, tc, Ub, part, fm_tile, rinv_b, A, up, chi_b);
     }
 }
 
@@ -371,14 +378,21 @@ static int launch_hydro_nr(cst_ctx* ctx, const double* U, double* A, const UpdAr
     const TileGeom tg = make_tile_geom(g);
     const size_t smem = 5ull * PART_COMP * sizeof(double);
     {   // per launch: the attribute belongs to the current device's instance of the kernel
-        if (cudaFuncSetAttribute(k_advect_hydro<NR>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
-            return CST_ECUDA;
+        const cudaError_t e = ctx->flatten
+            ? cudaFuncSetAttribute(k_advect_hydro<NR, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)
+            : cudaFuncSetAttribute(k_advect_hydro<NR, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return CST_ECUDA;
     }
     double* rinv = ctx->ws;
     double* Fm = ctx->ws + ws_rinv_doubles(g);
     // 32-byte loads of the x sweep need rows that start on 32-byte boundaries
     const bool x_vec = (g.nx % 4 == 0) && (((uintptr_t)U & 31) == 0);
-    k_advect_hydro<NR><<<(unsigned)tg.ntiles, NTHR, smem, st>>>(g, tg, U, A, rinv, Fm, up, x_vec);
+    if (ctx->flatten) {
+        const double* chi = Fm + ws_fm_doubles(g);
+        k_advect_hydro<NR, true><<<(unsigned)tg.ntiles, NTHR, smem, st>>>(g, tg, U, A, rinv, Fm, up, x_vec, chi);
+    } else {
+        k_advect_hydro<NR, false><<<(unsigned)tg.ntiles, NTHR, smem, st>>>(g, tg, U, A, rinv, Fm, up, x_vec, nullptr);
+    }
     ctx->launches++;
     return cudaGetLastError() == cudaSuccess ? CST_OK : CST_ECUDA;
 }

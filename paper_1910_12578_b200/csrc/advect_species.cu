@@ -27,12 +27,13 @@
 #define SP_TILE (TILE * TILE * SP_PITCH)
 
 // --------------------------------------------------------------------------- any tile extent ----
-template <int D, int NR>
+template <int D, int NR, bool FLAT>
 __device__ __forceinline__ void species_sweep(const Geom& g, const TileCoord& tc, const double* __restrict__ Us,
                                               const double* __restrict__ rinv_b,
                                               const double* __restrict__ Xs, double* __restrict__ Ps,
                                               const double* __restrict__ fm_tile,
-                                              double* __restrict__ A, int c, const UpdArgs& up)
+                                              double* __restrict__ A, int c, const UpdArgs& up,
+                                              const double* __restrict__ chi_b)
 {
     const int ng = CST_NG;
     const int tid = threadIdx.x, a = tid & (TILE - 1), b = tid >> 4;
@@ -73,7 +74,8 @@ __device__ __forceinline__ void species_sweep(const Geom& g, const TileCoord& tc
         double qn;
         if (p < L) qn = Xs[s0 + p * sstride];
         else qn = (p == L) ? hhi[0] : (p == L + 1) ? hhi[1] : hhi[2];
-        w.push(qn);
+        if (FLAT) w.push_flat(qn, chi_b[z0 + (long long)(p - 2) * stride]);   // optional CW84 flattening of zone p-2
+        else w.push(qn);
         if (p >= 2) {
             const double fmc = fmn;                     // mass flux of face f = p-2
             if (p < L + 2) fmn = fm[(p - 1) * NTHR];
@@ -100,10 +102,10 @@ __device__ __forceinline__ void species_sweep(const Geom& g, const TileCoord& tc
     }
 }
 
-template <int NR>
+template <int NR, bool FLAT>
 __global__ void __launch_bounds__(NTHR, 2)
 k_advect_species(Geom g, TileGeom tg, const double* __restrict__ U, double* __restrict__ A,
-                 const double* __restrict__ rinv, const double* __restrict__ Fm, UpdArgs up)
+                 const double* __restrict__ rinv, const double* __restrict__ Fm, UpdArgs up, const double* __restrict__ chi)
 {
     extern __shared__ double sm[];
     double* Xs = sm;                    // X_s = rho X_s / rho of the tile core
@@ -113,6 +115,7 @@ k_advect_species(Geom g, TileGeom tg, const double* __restrict__ U, double* __re
     const double* Ub = U + (long long)tc.b * g.box_g;
     const double* rinv_b = rinv + (long long)tc.b * g.comp_g;
     const double* fm_tile = Fm + tc.tile * 3LL * (TILE + 1) * NTHR;
+    const double* chi_b = FLAT ? chi + (long long)tc.b * g.comp_g : nullptr;
     const int tid = threadIdx.x, ti = tid & (TILE - 1), tr = tid >> 4;   // tr = row group 0..15
     // ghosted index of the tile zone (i = ti, j = tr, k = 0); row n of this thread is k = n
     const long long zt = ((long long)(tc.k0 + ng) * g.ey + (tc.j0 + tr + ng)) * g.ex + (tc.i0 + ti + ng);
@@ -126,11 +129,11 @@ k_advect_species(Geom g, TileGeom tg, const double* __restrict__ U, double* __re
                 Xs[(k * TILE + tr) * SP_PITCH + ti] = Us[z] * rinv_b[z];
             }
         __syncthreads();
-        species_sweep<0, NR>(g, tc, Us, rinv_b, Xs, Ps, fm_tile, A, c, up);
+        species_sweep<0, NR, FLAT>(g, tc, Us, rinv_b, Xs, Ps, fm_tile, A, c, up, chi_b);
         __syncthreads();
-        species_sweep<1, NR>(g, tc, Us, rinv_b, Xs, Ps, fm_tile, A, c, up);
+        species_sweep<1, NR, FLAT>(g, tc, Us, rinv_b, Xs, Ps, fm_tile, A, c, up, chi_b);
         __syncthreads();
-        species_sweep<2, NR>(g, tc, Us, rinv_b, Xs, Ps, fm_tile, A, c, up);
+        species_sweep<2, NR, FLAT>(g, tc, Us, rinv_b, Xs, Ps, fm_tile, A, c, up, chi_b);
     }
 }
 
@@ -162,7 +165,7 @@ static int launch_species_nr(cst_ctx* ctx, const double* U, double* A, const Upd
     const bool vec_ok = ((((uintptr_t)U | (uintptr_t)A | (uintptr_t)up.U_next | (uintptr_t)up.P[0] |
                            (uintptr_t)up.P[1] | (uintptr_t)up.P[2] | (uintptr_t)rinv) & 15) == 0);
     const bool all_full = vec_ok && (g.nx % TILE == 0) && (g.ny % TILE == 0) && (g.nz % TILE == 0);
-    bool tma = all_full;
+    bool tma = all_full && !ctx->flatten;              // flattening runs on the general kernel
     SptMaps maps;
     if (tma) {
         const unsigned long long nbv = (unsigned long long)g.nbox * g.nvar;
@@ -180,9 +183,15 @@ static int launch_species_nr(cst_ctx* ctx, const double* U, double* A, const Upd
         k_advect_species_tma<NR><<<(unsigned)(tg.ntiles * split), NTHR, SPT_SMEM, st>>>(g, tg, maps, U, A, rinv, Fm, up, split);
     } else {
         const size_t smem = 2ull * SP_TILE * sizeof(double);
-        if (cudaFuncSetAttribute(k_advect_species<NR>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
-            return CST_ECUDA;
-        k_advect_species<NR><<<(unsigned)tg.ntiles, NTHR, smem, st>>>(g, tg, U, A, rinv, Fm, up);
+        if (ctx->flatten) {
+            if (cudaFuncSetAttribute(k_advect_species<NR, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
+                return CST_ECUDA;
+            k_advect_species<NR, true><<<(unsigned)tg.ntiles, NTHR, smem, st>>>(g, tg, U, A, rinv, Fm, up, Fm + ws_fm_doubles(g));
+        } else {
+            if (cudaFuncSetAttribute(k_advect_species<NR, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
+                return CST_ECUDA;
+            k_advect_species<NR, false><<<(unsigned)tg.ntiles, NTHR, smem, st>>>(g, tg, U, A, rinv, Fm, up, nullptr);
+        }
     }
     ctx->launches++;
     return cudaGetLastError() == cudaSuccess ? CST_OK : CST_ECUDA;

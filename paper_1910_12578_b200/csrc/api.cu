@@ -66,6 +66,7 @@ extern "C" int cst_create(const cst_params* p, cst_ctx** out)
     c->xplan = nullptr;
     c->has_react = 0;
     c->diff_kth = 0.0; c->diff_cv = 1.0;
+    c->flatten = 0;
     for (int n = 0; n < 3; ++n) c->ev[n] = nullptr;
     int dev = 0;
     cudaError_t e = cudaGetDevice(&dev);
@@ -88,12 +89,12 @@ extern "C" int cst_destroy(cst_ctx* c)
 
 extern "C" long long cst_workspace_bytes(const cst_ctx* c)
 {
-    return c ? workspace_bytes(c->g) : -1;
+    return c ? workspace_bytes(c) : -1;
 }
 
 extern "C" int cst_set_workspace(cst_ctx* c, void* ws, long long bytes)
 {
-    if (!c || !ws || bytes < workspace_bytes(c->g) || ((uintptr_t)ws & 15)) return CST_EINVAL;
+    if (!c || !ws || bytes < workspace_bytes(c) || ((uintptr_t)ws & 15)) return CST_EINVAL;
     c->ws = (double*)ws; c->ws_bytes = bytes;
     return CST_OK;
 }
@@ -211,6 +212,13 @@ extern "C" int cst_step_host(cst_ctx* c, const double* U_host, double* A_host, d
     if (e == cudaSuccess) e = cudaMemcpyAsync(U_next_host, U_next_dev, ub, cudaMemcpyDeviceToHost, st);
     if (e == cudaSuccess) e = cudaStreamSynchronize(st);
     return e == cudaSuccess ? CST_OK : cuda_fail(e);
+}
+
+extern "C" int cst_set_flattening(cst_ctx* c, int on)
+{
+    if (!c) return CST_EINVAL;
+    c->flatten = on ? 1 : 0;
+    return CST_OK;
 }
 
 extern "C" int cst_set_diffusion(cst_ctx* c, double kth, double cv)

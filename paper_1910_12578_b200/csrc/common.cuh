@@ -40,6 +40,7 @@ struct cst_ctx {
     struct XPlan* xplan;     // cst_set_sublattice: ghost-exchange plan with the neighbouring ranks (exchange.cu)
     cst_react_params react;  // cst_set_reactions (react.cu)
     int has_react;
+    int flatten;             // cst_set_flattening (flatten.cu): chi array behind rinv and Fm in the workspace
     double diff_kth, diff_cv;  // cst_set_diffusion (diffuse.cu); kth = 0: no diffusion term
 };
 
@@ -65,11 +66,12 @@ int launch_advance_A(cst_ctx*, const double* U, double* A, double* U_next, doubl
                      const double* A_old_m, const QuadArgs& q, bool fused, cudaStream_t);
 int launch_advect_hydro(cst_ctx*, const double* U, double* A, const UpdArgs& up, cudaStream_t);
 int launch_advect_species(cst_ctx*, const double* U, double* A, const UpdArgs& up, cudaStream_t);
-long long workspace_bytes(const Geom& g);
+long long workspace_bytes(const cst_ctx* ctx);
 int launch_sdc_update(cst_ctx*, double* U_next, const double* U_m, double dt_m,
                       const double* A_new_m, const double* A_old_m, const QuadArgs& q, cudaStream_t);
 int launch_cfl(cst_ctx*, const double* U, double cfl, double* dt_out_dev, cudaStream_t);
 int launch_validate(cst_ctx*, const double* U, cudaStream_t);   // count left in d_scratch[2]
+int launch_flatten(cst_ctx*, const double* U, cudaStream_t);   // flatten.cu: chi of every zone -1 .. n -> workspace
 // diffuse.cu: A[rho E] += k_th lap T (and U_next[rho E] += ca * that when U_next != nullptr)
 int launch_diffuse_add(cst_ctx*, const double* U, double* A, double* U_next, double ca, cudaStream_t);
 // react.cu: R != 0

@@ -48,4 +48,18 @@ struct PpmWindow {
         qm = a; qp = b;
         q2 = q1; q1 = qn; dq1 = dqn; s2 = s1; e = en;
     }
+    // push with CW84 shock flattening (flatten.cu, reading F4): the parabola of zone p-2 that this step completes is
+    // blended with the zone average, q+- <- chi q+- + (1 - chi) q, chi = the coefficient of zone p-2 (chi = 1: unchanged)
+    __device__ __forceinline__ void push_flat(double qn, double chi)
+    {
+        qpL = qp;
+        const double dqn = qn - q1;
+        const double s1 = slope2(dq1, dqn);
+        const double en = edge_value(q2, dq1, s2, s1);
+        double a = e, b = en;
+        monotonize(q2, a, b);
+        const double rest = (1.0 - chi) * q2;
+        qm = fma(chi, a, rest); qp = fma(chi, b, rest);
+        q2 = q1; q1 = qn; dq1 = dqn; s2 = s1; e = en;
+    }
 };
