@@ -42,6 +42,9 @@ def lib():
         _lib.orc_fill_ghosts.argtypes = [P, _dp]
         _lib.orc_advance_A.argtypes = [P, _dp, _dp]
         _lib.orc_advance_A_flat.argtypes = [P, _dp, _dp]
+        _lib.orc_advance_A4.argtypes = [P, _dp, _dp]
+        _lib.orc_ppm4_line.argtypes = [C.c_int, _dp, _dp, _dp]
+        _lib.orc_ppm4_line.restype = None
         _lib.orc_flatten_line.argtypes = [C.c_int, _dp, _dp, C.c_double, _dp]
         _lib.orc_flatten_line.restype = None
         _lib.orc_sdc_update.argtypes = [P, _dp, _dp, C.c_double, _dp, _dp, C.c_int,
@@ -126,6 +129,23 @@ def advance_A_flat(cfg, U, A=None):
         A = np.empty(a_shape(cfg), dtype=np.float64)
     _chk(lib().orc_advance_A_flat(C.byref(make_params(cfg)), _ptr(U), _ptr(A)), "advance_A_flat")
     return A
+
+
+def advance_A4(cfg, U, A=None):
+    """Fourth-order finite-volume <A(U)> (oracle/orc_fourth.c, readings G1-G9); the whole ghost shell must be filled."""
+    assert U.shape == u_shape(cfg)
+    if A is None:
+        A = np.empty(a_shape(cfg), dtype=np.float64)
+    _chk(lib().orc_advance_A4(C.byref(make_params(cfg)), _ptr(U), _ptr(A)), "advance_A4")
+    return A
+
+
+def ppm4_line(q):
+    """Limited fourth-order parabola edges (qm, qp) of one line of cell averages; valid for zones 2..n-3."""
+    q = np.ascontiguousarray(q, dtype=np.float64)
+    qm, qp = np.full_like(q, np.nan), np.full_like(q, np.nan)
+    lib().orc_ppm4_line(len(q), _ptr(q), _ptr(qm), _ptr(qp))
+    return qm, qp
 
 
 def flatten_line(p, u, small_pres=1e-200):
