@@ -126,6 +126,18 @@ int cst_sdc_update(cst_ctx* ctx, double* U_next, const double* U_m, double dt_m,
                    const double* A_new_m, const double* A_old_m,
                    int nquad, const double* const* A_quad, const double* w_quad, void* stream);
 
+/* Spatial order of <A(U)> ("a fourth-order method in space and time (using a Simpsons rule for the integral and
+ * the spatial reconstruction of [12])"; readings G1-G9).  order = 2 (default, the graded
+ * path): PPM + CW84 limiter as described at cst_advance_A.  order = 4: U and A are CELL AVERAGES and every later
+ * cst_advance_A / cst_advance_A_update / cst_step_host evaluates the fourth-order finite-volume operator -- cell-centre
+ * and cell-average primitives through undivided Laplacians / 24, (7/12, -1/12) face averages with the
+ * extremum-preserving limiter of [12] (McCorquodale & Colella 2011; without its third-difference test, whose stencil
+ * needs a fifth ghost zone), face-centred states, two HLLC solves per face and transverse Laplacians of the fluxes.
+ * It reads the WHOLE 4-deep ghost shell; together with the 3-node Simpson weights of cst_sdc_update it is the paper's
+ * fourth-order scheme.  The workspace is larger (cst_workspace_bytes(): about 5 NVAR doubles per zone): set the order
+ * BEFORE sizing / setting the workspace.  Flattening does not apply to order 4.  CST_EINVAL: order not 2 or 4. */
+int cst_set_order(cst_ctx* ctx, int order);
+
 /* Shock flattening (Colella & Woodward 1984, appendix; P:L52 ref [15]; DESIGN.md readings
  * F1-F4), an option that is OFF by default (the graded path, Q4).  With on != 0 every later
  * cst_advance_A / cst_advance_A_update / cst_step_host first computes the flattening coefficient chi of every zone

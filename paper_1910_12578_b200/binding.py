@@ -15,7 +15,7 @@ EXPORTS = ["cst_create", "cst_destroy", "cst_workspace_bytes", "cst_set_workspac
            "cst_advance_A_update", "cst_cfl_dt_device", "cst_cfl_dt", "cst_validate", "cst_step_host",
            "cst_set_timing", "cst_last_advance_ms", "cst_launch_count", "cst_strerror", "cst_version",
            "cst_debug_rcp_sqrt", "cst_debug_tile_count", "cst_debug_tile_map",
-           "cst_set_flattening", "cst_set_diffusion", "cst_set_reactions", "cst_react_R", "cst_sdc_update_react", "cst_react_failures",
+           "cst_set_order", "cst_set_flattening", "cst_set_diffusion", "cst_set_reactions", "cst_react_R", "cst_sdc_update_react", "cst_react_failures",
            "cst_exchange_plan", "cst_set_sublattice", "cst_exchange_info", "cst_exchange_pack", "cst_exchange_unpack"]
 
 
@@ -85,6 +85,7 @@ def load():
     lib.cst_debug_tile_map.argtypes = [_vp, _vp, _vp]
     lib.cst_launch_count.argtypes = [_vp]
     lib.cst_launch_count.restype = C.c_longlong
+    lib.cst_set_order.argtypes = [_vp, C.c_int]
     lib.cst_set_flattening.argtypes = [_vp, C.c_int]
     lib.cst_set_diffusion.argtypes = [_vp, C.c_double, C.c_double]
     lib.cst_set_reactions.argtypes = [_vp, C.POINTER(CstReactParams)]
@@ -235,6 +236,10 @@ class Context:
         self._check(self.lib.cst_step_host(self._h, _ptr(U_host), _ptr(A_host), _ptr(U_next_host), _ptr(U_dev),
                                            _ptr(U_next_dev), _ptr(A_dev), float(dt_m), _stream(stream)),
                     "cst_step_host")
+
+    def set_order(self, order):
+        """Spatial order of <A(U)>: 2 (default) or 4; changes workspace_bytes(): set the workspace afterwards."""
+        self._check(self.lib.cst_set_order(self._h, int(order)), "cst_set_order")
 
     def set_flattening(self, on):
         """Switch CW84 shock flattening on / off; enlarges workspace_bytes(): set the workspace afterwards."""

@@ -7,8 +7,9 @@
 #include "tile.cuh"
 
 long long workspace_bytes(const cst_ctx* ctx)
-{   // [rinv][Fm] and, with flattening switched on, [chi] (one double per ghosted zone)
+{   // [rinv][Fm] and, with flattening switched on, [chi] (one double per ghosted zone); order 4: fourth.cu's arrays
     const Geom& g = ctx->g;
+    if (ctx->order == 4) return fourth_workspace_doubles(g) * (long long)sizeof(double);
     return (ws_rinv_doubles(g) + ws_fm_doubles(g) + (ctx->flatten ? ws_rinv_doubles(g) : 0)) * (long long)sizeof(double);
 }
 
@@ -40,6 +41,12 @@ int launch_advance_A(cst_ctx* ctx, const double* U, double* A, double* U_next, d
     bool split = false;
     if (fused && !make_upd(up, U, A, U_next, dt_m, A_old_m, q)) { up.nr = -1; split = true; }
     int rc = CST_OK;
+    if (ctx->order == 4) {             // fourth-order <A(U)> (fourth.cu), then the optional extra term and the plain node update
+        rc = launch_advance_A4(ctx, U, A, st);
+        if (!rc && ctx->diff_kth != 0.0) rc = launch_diffuse_add(ctx, U, A, nullptr, 0.0, st);
+        if (rc || !fused) return rc;
+        return launch_sdc_update(ctx, U_next, U, dt_m, A, A_old_m, q, st);
+    }
     if (ctx->flatten && (rc = launch_flatten(ctx, U, st)) != CST_OK) return rc;
     if (ctx->timing) cudaEventRecord(ctx->ev[0], st);
     rc = launch_advect_hydro(ctx, U, A, up, st);

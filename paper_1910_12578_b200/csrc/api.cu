@@ -67,6 +67,7 @@ extern "C" int cst_create(const cst_params* p, cst_ctx** out)
     c->has_react = 0;
     c->diff_kth = 0.0; c->diff_cv = 1.0;
     c->flatten = 0;
+    c->order = 2;
     for (int n = 0; n < 3; ++n) c->ev[n] = nullptr;
     int dev = 0;
     cudaError_t e = cudaGetDevice(&dev);
@@ -212,6 +213,13 @@ extern "C" int cst_step_host(cst_ctx* c, const double* U_host, double* A_host, d
     if (e == cudaSuccess) e = cudaMemcpyAsync(U_next_host, U_next_dev, ub, cudaMemcpyDeviceToHost, st);
     if (e == cudaSuccess) e = cudaStreamSynchronize(st);
     return e == cudaSuccess ? CST_OK : cuda_fail(e);
+}
+
+extern "C" int cst_set_order(cst_ctx* c, int order)
+{
+    if (!c || (order != 2 && order != 4)) return CST_EINVAL;
+    c->order = order;
+    return CST_OK;
 }
 
 extern "C" int cst_set_flattening(cst_ctx* c, int on)

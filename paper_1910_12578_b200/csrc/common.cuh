@@ -40,6 +40,7 @@ struct cst_ctx {
     struct XPlan* xplan;     // cst_set_sublattice: ghost-exchange plan with the neighbouring ranks (exchange.cu)
     cst_react_params react;  // cst_set_reactions (react.cu)
     int has_react;
+    int order;               // cst_set_order: 2 (PPM path, default) or 4 (fourth.cu)
     int flatten;             // cst_set_flattening (flatten.cu): chi array behind rinv and Fm in the workspace
     double diff_kth, diff_cv;  // cst_set_diffusion (diffuse.cu); kth = 0: no diffusion term
 };
@@ -71,6 +72,8 @@ int launch_sdc_update(cst_ctx*, double* U_next, const double* U_m, double dt_m,
                       const double* A_new_m, const double* A_old_m, const QuadArgs& q, cudaStream_t);
 int launch_cfl(cst_ctx*, const double* U, double cfl, double* dt_out_dev, cudaStream_t);
 int launch_validate(cst_ctx*, const double* U, cudaStream_t);   // count left in d_scratch[2]
+int launch_advance_A4(cst_ctx*, const double* U, double* A, cudaStream_t);   // fourth.cu: fourth-order <A(U)>
+long long fourth_workspace_doubles(const Geom& g);
 int launch_flatten(cst_ctx*, const double* U, cudaStream_t);   // flatten.cu: chi of every zone -1 .. n -> workspace
 // diffuse.cu: A[rho E] += k_th lap T (and U_next[rho E] += ca * that when U_next != nullptr)
 int launch_diffuse_add(cst_ctx*, const double* U, double* A, double* U_next, double ca, cudaStream_t);
