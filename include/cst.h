@@ -53,7 +53,7 @@ typedef struct {
 
 typedef struct cst_ctx cst_ctx;    /* opaque */
 
-/* Validates params (CST_EINVAL: NULL, ng != 4, n_d < ng, nspec out of range, more than 65535 boxes, non-positive
+/* Validates params (CST_EINVAL: NULL, ng != 4, n_d < ng, nspec out of range, more than 2^24 boxes, non-positive
  * widths, gamma <= 1, bad or one-sided-periodic BC) and allocates the context's scratch.
  * Range of the state: the kernels form products such as gamma*p*rho and use reciprocal / square-root sequences
  * without the special-case branches of the library routines, so rho and p (floors included) must stay within

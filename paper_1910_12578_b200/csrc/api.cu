@@ -24,7 +24,7 @@ static int validate(const cst_params* p)
     if (p->ng != CST_NG) return CST_EINVAL;
     if (p->nx < p->ng || p->ny < p->ng || p->nz < p->ng) return CST_EINVAL;
     if (p->nbx < 1 || p->nby < 1 || p->nbz < 1) return CST_EINVAL;
-    if ((long long)p->nbx * p->nby * p->nbz > 65535) return CST_EINVAL;
+    if ((long long)p->nbx * p->nby * p->nbz > (1 << 24)) return CST_EINVAL;
     if (p->nspec < 0 || p->nspec > CST_MAX_NSPEC) return CST_EINVAL;
     if (!(p->dx > 0) || !(p->dy > 0) || !(p->dz > 0) || !(p->gamma > 1)) return CST_EINVAL;
     for (int d = 0; d < 3; ++d) {

@@ -25,13 +25,13 @@ __device__ __forceinline__ int map_dir(int g, int D, int bc_lo, int bc_hi, bool&
 }
 
 __global__ void __launch_bounds__(256)
-k_fill_ghosts(Geom g, double* __restrict__ U, long long n0, long long n1, long long n2)
+k_fill_ghosts(Geom g, double* __restrict__ U, long long n0, long long n1, long long n2, unsigned blocks_per_box)
 {
     const int ng = CST_NG;
-    const int b = blockIdx.y;
+    const int b = blockIdx.x / blocks_per_box;          // 1-D grid: no limit on the number of boxes
     const int bi = b % g.nbx, bj = (b / g.nbx) % g.nby, bk = b / (g.nbx * g.nby);
     const long long ntot = n0 + n1 + n2;
-    const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const long long t = (long long)(blockIdx.x - (unsigned)b * blocks_per_box) * blockDim.x + threadIdx.x;
     if (t >= ntot) return;
     int i, j, k;
     if (t < n0) {                       // z slabs: all j, all i
@@ -93,9 +93,9 @@ int launch_fill_ghosts(cst_ctx* ctx, double* U, cudaStream_t st)
     const long long n1 = 2LL * ng * g.nz * g.ex;
     const long long n2 = 2LL * ng * (long long)g.nz * g.ny;
     const long long ntot = n0 + n1 + n2;
-    const long long nb = (ntot + 255) / 256;            // <= 2^31 - 1 blocks in x for any box that fits in memory
-    dim3 grid((unsigned)nb, (unsigned)g.nbox, 1);
-    k_fill_ghosts<<<grid, 256, 0, st>>>(g, U, n0, n1, n2);
+    const long long nb = (ntot + 255) / 256;
+    if (nb * g.nbox > 0x7fffffffLL) return CST_EINVAL;  // more ghost zones than any device memory holds
+    k_fill_ghosts<<<(unsigned)(nb * g.nbox), 256, 0, st>>>(g, U, n0, n1, n2, (unsigned)nb);
     ctx->launches++;
     return cudaGetLastError() == cudaSuccess ? CST_OK : CST_ECUDA;
 }

@@ -89,7 +89,7 @@ struct ReactQuad {           // quadrature arrays of A and R, passed by value
 __global__ void __launch_bounds__(128)
 k_sdc_update_react(Geom g, ReactDev r, double* U_next, const double* U_m, double dt,
                    const double* __restrict__ A_new, const double* __restrict__ A_old,
-                   const double* __restrict__ R_old_next, ReactQuad q, double* __restrict__ R_new,
+                   const double* R_old_next, ReactQuad q, double* R_new,      // may be the same array (cst.h)
                    unsigned long long* __restrict__ n_fail)
 {
     const int ng = CST_NG;

@@ -70,6 +70,7 @@ def test_A4_matches_oracle(n, nb, ns, bc, state):
     ctx.advance_A(Ud, Ad)
     eA = comp_err(Ad.cpu().numpy(), Ao)
     assert eA.max() <= TOL, eA
+    print("A4 error", eA.max())
     # the "fused" call: A4 followed by the plain node update
     dt = 0.3 * orc.cfl_dt(cfg, U, 0.5)
     rng = np.random.default_rng(5)
