@@ -45,6 +45,7 @@ def parse():
     ap.add_argument("--workload", type=int, default=None, choices=[0, 1, 2, 3, 4],
                     help="time this config only (default: configs[3], then configs[4] under \"also\")")
     ap.add_argument("--n", type=int, default=None, help="override zones per box side (debug only; marks the line)")
+    ap.add_argument("--no-tune", action="store_true", help="keep species-kernel variant 0 instead of timing the variants")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     return ap.parse_args()
@@ -274,6 +275,18 @@ def measure(cfg, args, rank, world, local, dev, want_e2e, want_cpu_baseline):
     A_old1.copy_(A_old0).mul_(0.9)
     w = [0.5 * dt, 0.5 * dt]
 
+    # kernel variants of the species half (cst_tune_advance): every variant is timed on these buffers before the
+    # warm-up steps and the fastest is kept; all variants give bit-identical results (tests/test_gpu_variants.py)
+    tuned = {"species_variant": 0, "ms": None, "note": "not tuned"}
+    if not getattr(args, "no_tune", False) and N > 5:
+        try:
+            v, ms_v = ctx.tune_advance(U, A_new, U_next, dt, A_old0, [A_old0, A_old1], w, repeats=2)
+            tuned = {"species_variant": v, "ms": ms_v, "note": "cst_tune_advance: fused advance (hydro + species kernels), "
+                     "min of 2 runs per variant"}
+        except Exception as exc:
+            ctx.set_variant(0)
+            tuned = {"species_variant": 0, "ms": None, "note": f"tuning failed ({exc}); variant 0"}
+
     ev = lambda: torch.cuda.Event(enable_timing=True)
     k_ev, k_ms2 = [], []
     ctx.set_timing(True)      # CUDA events around the two kernels of the advance, on this stream (cst.h)
@@ -334,8 +347,13 @@ def measure(cfg, args, rank, world, local, dev, want_e2e, want_cpu_baseline):
         traffic = prof.get("k_advect_species_dram_bytes_per_launch")
     except Exception:
         pass
+    if tuned["species_variant"] != 0 or args.n:
+        # the ncu annotations were captured on variant 0 of the species kernel at full size: they do not describe this run
+        traffic = None
+        prof = {k: v for k, v in prof.items() if "species" not in k}
     if N > 5:
-        dom, dom_ms, dom_bytes = "k_advect_species_tma<2> (S1-S5, species components)", ms_species, ab["advance_species"]
+        vname = "k_advect_species_tma<2>" if tuned["species_variant"] == 0 else f"k_advect_species_tma_v<2, {tuned['species_variant']}>"
+        dom, dom_ms, dom_bytes = f"{vname} (S1-S5, species components)", ms_species, ab["advance_species"]
     else:
         dom, dom_ms, dom_bytes = "k_advect_hydro<2> (S1-S5, hydro components)", ms_hydro, ab["advance_hydro"]
     achieved = dom_bytes * zones / (dom_ms * 1e-3) / 1e9
@@ -358,7 +376,7 @@ def measure(cfg, args, rank, world, local, dev, want_e2e, want_cpu_baseline):
     sm_hz = (clocks or {}).get("sm_mhz") or 1965.0
     issue_peak = ctx_sm_count * 4 * sm_hz * 1e6
     fp64_peak = ctx_sm_count * 64 * sm_hz * 1e6
-    if prof.get("k_advect_species_warp_instr_per_launch"):
+    if prof.get("k_advect_species_warp_instr_per_launch") and prof.get("k_advect_hydro_warp_instr_per_launch"):
         roofline["issue"] = {
             "k_advect_species_issue_frac": prof["k_advect_species_warp_instr_per_launch"] / (ms_species * 1e-3) / issue_peak,
             "k_advect_hydro_issue_frac": prof["k_advect_hydro_warp_instr_per_launch"] / (ms_hydro * 1e-3) / issue_peak,
@@ -430,7 +448,7 @@ def measure(cfg, args, rank, world, local, dev, want_e2e, want_cpu_baseline):
                            "parallelism": f"box lattice sharded over {world} ranks, bricks {part[0]}x{part[1]}x{part[2]}" if world > 1
                                           else "single GPU",
                            "ms_per_step_best": float(min(per_step)), "ms_per_step_median": float(np.median(per_step)),
-                           "debug_size_override": bool(args.n)},
+                           "tuned": tuned, "debug_size_override": bool(args.n)},
                 "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline,
                 "cpu_baseline": cpu_baseline}
     ctx.destroy()

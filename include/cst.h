@@ -126,6 +126,23 @@ int cst_sdc_update(cst_ctx* ctx, double* U_next, const double* U_m, double dt_m,
                    const double* A_new_m, const double* A_old_m,
                    int nquad, const double* const* A_quad, const double* w_quad, void* stream);
 
+/* Kernel variants of the species half of <A(U)> on boxes made of full 16^3 tiles (csrc/species_tma.cuh); every variant
+ * performs the same operations in the same order, so results are bit-identical.
+ *   0  (default) conversion phase + three sweeps + write-out phase per species: the kernel that has been profiled;
+ *   1  X = rho X / rho formed inside the x sweep (no conversion phase);
+ *   2  as 1, and each component is written out from its own z sweep (no write-out phase).
+ * cst_set_variant selects one (CST_EINVAL outside 0..2); cst_get_variant returns the current one.
+ * cst_tune_advance runs cst_advance_A_update (same arguments, same rules) `repeats` + 1 times with every variant on
+ * the caller's buffers, times each with CUDA events on `stream` (minimum over the repeats; the first run of a variant
+ * is a warm-up), keeps the fastest for all later calls and leaves A_new_m / U_next valid; ms_out (HOST, 3 floats, may
+ * be NULL) receives the times in milliseconds.  Synchronises the stream.  Measurement, not arithmetic: which variant
+ * wins depends on the device and the box shape. */
+int cst_set_variant(cst_ctx* ctx, int species_variant);
+int cst_get_variant(const cst_ctx* ctx);
+int cst_tune_advance(cst_ctx* ctx, const double* U_m, double* A_new_m, double* U_next, double dt_m,
+                     const double* A_old_m, int nquad, const double* const* A_quad, const double* w_quad,
+                     int repeats, float* ms_out, void* stream);
+
 /* Spatial order of <A(U)> ("a fourth-order method in space and time (using a Simpsons rule for the integral and
  * the spatial reconstruction of [12])"; readings G1-G9).  order = 2 (default, the graded
  * path): PPM + CW84 limiter as described at cst_advance_A.  order = 4: U and A are CELL AVERAGES and every later

@@ -154,6 +154,21 @@ k_advect_species_tma(const Geom g, const TileGeom tg, const __grid_constant__ Sp
                  Fm + tc.tile * 3LL * (TILE + 1) * NTHR, A, up, sm, s_begin, s_end);
 }
 
+// the variant kernels (species_tma.cuh spt_tile_v; cst_set_variant / cst_tune_advance): same arithmetic, fewer phases
+template <int NR, int V>
+__global__ void __launch_bounds__(NTHR, 2)
+k_advect_species_tma_v(const Geom g, const TileGeom tg, const __grid_constant__ SptMaps maps, const double* __restrict__ U,
+                       double* __restrict__ A, const double* __restrict__ rinv, const double* __restrict__ Fm,
+                       const UpdArgs up, const int split)
+{
+    extern __shared__ __align__(128) double sm[];
+    const int part = blockIdx.x % split;
+    const TileCoord tc = tile_coord(g, tg, blockIdx.x / split);
+    const int s_begin = (int)((long long)g.nspec * part / split), s_end = (int)((long long)g.nspec * (part + 1) / split);
+    spt_tile_v<NR, V>(g, tc, maps, U + (long long)tc.b * g.box_g, rinv + (long long)tc.b * g.comp_g,
+                      Fm + tc.tile * 3LL * (TILE + 1) * NTHR, A, up, sm, s_begin, s_end);
+}
+
 template <int NR>
 static int launch_species_nr(cst_ctx* ctx, const double* U, double* A, const UpdArgs& up, cudaStream_t st)
 {
@@ -180,7 +195,18 @@ static int launch_species_nr(cst_ctx* ctx, const double* U, double* A, const Upd
         if (cudaFuncSetAttribute(k_advect_species_tma<NR>, cudaFuncAttributeMaxDynamicSharedMemorySize, SPT_SMEM) != cudaSuccess)
             return CST_ECUDA;
         const int split = g.nspec < SPT_SPLIT ? g.nspec : SPT_SPLIT;
-        k_advect_species_tma<NR><<<(unsigned)(tg.ntiles * split), NTHR, SPT_SMEM, st>>>(g, tg, maps, U, A, rinv, Fm, up, split);
+        const unsigned grid = (unsigned)(tg.ntiles * split);
+        if (ctx->species_variant == 1) {
+            if (cudaFuncSetAttribute(k_advect_species_tma_v<NR, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, SPT_SMEM) != cudaSuccess)
+                return CST_ECUDA;
+            k_advect_species_tma_v<NR, 1><<<grid, NTHR, SPT_SMEM, st>>>(g, tg, maps, U, A, rinv, Fm, up, split);
+        } else if (ctx->species_variant == 2) {
+            if (cudaFuncSetAttribute(k_advect_species_tma_v<NR, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, SPT_SMEM) != cudaSuccess)
+                return CST_ECUDA;
+            k_advect_species_tma_v<NR, 2><<<grid, NTHR, SPT_SMEM, st>>>(g, tg, maps, U, A, rinv, Fm, up, split);
+        } else {
+            k_advect_species_tma<NR><<<grid, NTHR, SPT_SMEM, st>>>(g, tg, maps, U, A, rinv, Fm, up, split);
+        }
     } else {
         const size_t smem = 2ull * SP_TILE * sizeof(double);
         if (ctx->flatten) {

@@ -68,6 +68,7 @@ extern "C" int cst_create(const cst_params* p, cst_ctx** out)
     c->diff_kth = 0.0; c->diff_cv = 1.0;
     c->flatten = 0;
     c->order = 2;
+    c->species_variant = 0;
     for (int n = 0; n < 3; ++n) c->ev[n] = nullptr;
     int dev = 0;
     cudaError_t e = cudaGetDevice(&dev);
@@ -213,6 +214,55 @@ extern "C" int cst_step_host(cst_ctx* c, const double* U_host, double* A_host, d
     if (e == cudaSuccess) e = cudaMemcpyAsync(U_next_host, U_next_dev, ub, cudaMemcpyDeviceToHost, st);
     if (e == cudaSuccess) e = cudaStreamSynchronize(st);
     return e == cudaSuccess ? CST_OK : cuda_fail(e);
+}
+
+extern "C" int cst_set_variant(cst_ctx* c, int species_variant)
+{
+    if (!c || species_variant < 0 || species_variant > 2) return CST_EINVAL;
+    c->species_variant = species_variant;
+    return CST_OK;
+}
+
+extern "C" int cst_get_variant(const cst_ctx* c) { return c ? c->species_variant : CST_EINVAL; }
+
+// Times the fused advance with every species-kernel variant on the caller's own buffers and keeps the fastest.
+extern "C" int cst_tune_advance(cst_ctx* c, const double* U_m, double* A_new_m, double* U_next, double dt_m,
+                                const double* A_old_m, int nquad, const double* const* A_quad, const double* w_quad,
+                                int repeats, float* ms_out, void* stream)
+{
+    if (!c || repeats < 1) return CST_EINVAL;
+    cudaStream_t st = (cudaStream_t)stream;
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) {
+        if (e0) cudaEventDestroy(e0);
+        return cuda_fail(cudaGetLastError());
+    }
+    const int keep_timing = c->timing;
+    c->timing = 0;
+    int best = 0, rc = CST_OK;
+    float best_ms = 0.f;
+    for (int v = 0; v <= 2 && rc == CST_OK; ++v) {
+        c->species_variant = v;
+        float ms_v = 0.f;
+        for (int n = 0; n <= repeats && rc == CST_OK; ++n) {          // the first run of a variant is a warm-up
+            cudaEventRecord(e0, st);
+            rc = cst_advance_A_update(c, U_m, A_new_m, U_next, dt_m, A_old_m, nquad, A_quad, w_quad, stream);
+            cudaEventRecord(e1, st);
+            if (rc != CST_OK) break;
+            if (cudaEventSynchronize(e1) != cudaSuccess) { rc = cuda_fail(cudaGetLastError()); break; }
+            float ms = 0.f;
+            cudaEventElapsedTime(&ms, e0, e1);
+            if (n == 1 || (n > 1 && ms < ms_v)) ms_v = ms;
+        }
+        if (ms_out) ms_out[v] = ms_v;
+        if (v == 0 || ms_v < best_ms) { best = v; best_ms = ms_v; }
+    }
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
+    c->timing = keep_timing;
+    c->species_variant = (rc == CST_OK) ? best : 0;
+    if (rc == CST_OK && best != 2)      // leave the outputs as the chosen kernel writes them (all variants agree bit for bit)
+        rc = cst_advance_A_update(c, U_m, A_new_m, U_next, dt_m, A_old_m, nquad, A_quad, w_quad, stream);
+    return rc;
 }
 
 extern "C" int cst_set_order(cst_ctx* c, int order)

@@ -73,6 +73,11 @@ __device__ __forceinline__ void spt_stg2(double* a, double2 v, unsigned long lon
     asm volatile("st.global.L2::cache_hint.v2.f64 [%0], {%1,%2}, %3;" :: "l"(a), "d"(v.x), "d"(v.y), "l"(pol) : "memory");
 }
 
+__device__ __forceinline__ void spt_stg(double* a, double v, unsigned long long pol)
+{
+    asm volatile("st.global.L2::cache_hint.f64 [%0], %1, %2;" :: "l"(a), "d"(v), "l"(pol) : "memory");
+}
+
 // Pencil of this thread in direction D: (a, b) = (tid % 16, tid / 16) = (j, k) | (i, k) | (i, j).
 // X tile: zone (k, j, x) at k * SPT_XPLANE + j * SPT_XW + (x + 4), x = -4 .. 19; P tile: zone (k, j, i) at
 // k * SPT_PLANE + j * SPT_PITCH + i.
@@ -216,6 +221,164 @@ __device__ __forceinline__ void spt_sweep_x(const double* __restrict__ Xr, doubl
         w.push(xe.y); F = spt_face(w, fn[1]); hold = fma(F - Fprev, nrd, 0.0); Fprev = F;
         w.push(xf.x); F = spt_face(w, fn[2]); z = fma(F - Fprev, nrd, 0.0);
         *reinterpret_cast<double2*>(Pp + 14) = make_double2(hold, z);
+    }
+}
+
+// ---- variant kernels (cst_set_variant; species_tile V = 1, 2): the same arithmetic with fewer phases per species ----
+// x sweep that also forms X = rho X / rho: the pencil's row of the raw tile (24 values, halos included) is multiplied by
+// the row of 1/rho (twelve 16-byte loads requested up front, consumed in pencil order), fed to the window, and the core
+// pairs are written back in place for the y / z sweeps.  Replaces spt_convert (one phase, one dependent round of L2
+// loads and 2 x 48 KB of shared-memory traffic per species).  Same products, same order: results are bit-identical.
+__device__ __forceinline__ double2 spt_conv_pair(double* __restrict__ Xr, const int o, const double2 r, const bool core)
+{   // X of the two positions at row offset o; core pairs go back to the tile for the y / z sweeps
+    double2 v = *reinterpret_cast<const double2*>(Xr + o);
+    v.x *= r.x; v.y *= r.y;
+    if (core) *reinterpret_cast<double2*>(Xr + o) = v;
+    return v;
+}
+__device__ __forceinline__ void spt_sweep_x_conv(double* __restrict__ Xr, double* __restrict__ Pp, const double* __restrict__ fm,
+                                                 const double* __restrict__ rrow, const double nrd, const unsigned long long keep)
+{
+    PpmWindow w;
+    const double2 r0 = spt_ldg2(rrow, keep), r1 = spt_ldg2(rrow + 2, keep), r2 = spt_ldg2(rrow + 4, keep), r3 = spt_ldg2(rrow + 6, keep);
+    double2 rn0 = spt_ldg2(rrow + 8, keep), rn1 = spt_ldg2(rrow + 10, keep);     // 1/rho of the next group of four
+    double fn[4], fnn[4];
+    const double f0 = spt_ldg(fm, keep), f1 = spt_ldg(fm + NTHR, keep);
+#pragma unroll
+    for (int e = 0; e < 4; ++e) fn[e] = spt_ldg(fm + (2 + e) * NTHR, keep);
+#pragma unroll
+    for (int e = 0; e < 4; ++e) fnn[e] = spt_ldg(fm + (6 + e) * NTHR, keep);
+    const double2 h0 = spt_conv_pair(Xr, 0, r0, false), h1 = spt_conv_pair(Xr, 2, r1, false);
+    const double2 xa = spt_conv_pair(Xr, 4, r2, true), xb = spt_conv_pair(Xr, 6, r3, true);
+    w.start(h0.y); w.warm1(h1.x); w.warm2(h1.y);
+    w.warm3(xa.x);
+    w.push(xa.y);
+    w.push(xb.x);
+    const double F0 = spt_face(w, f0);
+    w.push(xb.y);
+    double Fprev = spt_face(w, f1);
+    double pend = fma(Fprev - F0, nrd, 0.0);                    // zone 0, stored with zone 1
+#pragma unroll 1
+    for (int it = 1; it <= 3; ++it) {                 // positions 4it .. 4it+3: faces 4it-2 .., zones 4it-3 ..
+        double fc[4];
+#pragma unroll
+        for (int e = 0; e < 4; ++e) {
+            fc[e] = fn[e];
+            fn[e] = fnn[e];
+            if (it < 2 || (it == 2 && e < 3)) fnn[e] = spt_ldg(fm + (4 * it + 6 + e) * NTHR, keep);
+        }
+        const double2 rc0 = rn0, rc1 = rn1;
+        rn0 = spt_ldg2(rrow + 8 + 4 * it, keep); rn1 = spt_ldg2(rrow + 10 + 4 * it, keep);   // it = 3: the pairs of the tail
+        const double2 xc = spt_conv_pair(Xr, 4 + 4 * it, rc0, true), xd = spt_conv_pair(Xr, 6 + 4 * it, rc1, true);
+        double* __restrict__ pg = Pp + 4 * it - 4;                 // zones 4it-4 .. 4it-1 are complete after this group
+        double F, z, hold;
+        w.push(xc.x); F = spt_face(w, fc[0]); z = fma(F - Fprev, nrd, 0.0); Fprev = F;
+        *reinterpret_cast<double2*>(pg) = make_double2(pend, z);
+        w.push(xc.y); F = spt_face(w, fc[1]); hold = fma(F - Fprev, nrd, 0.0); Fprev = F;
+        w.push(xd.x); F = spt_face(w, fc[2]); z = fma(F - Fprev, nrd, 0.0); Fprev = F;
+        *reinterpret_cast<double2*>(pg + 2) = make_double2(hold, z);
+        w.push(xd.y); F = spt_face(w, fc[3]); pend = fma(F - Fprev, nrd, 0.0); Fprev = F;
+    }
+    {
+        const double2 xe = spt_conv_pair(Xr, 20, rn0, false), xf = spt_conv_pair(Xr, 22, rn1, false);
+        double F, z, hold;
+        w.push(xe.x); F = spt_face(w, fn[0]); z = fma(F - Fprev, nrd, 0.0); Fprev = F;
+        *reinterpret_cast<double2*>(Pp + 12) = make_double2(pend, z);
+        w.push(xe.y); F = spt_face(w, fn[1]); hold = fma(F - Fprev, nrd, 0.0); Fprev = F;
+        w.push(xf.x); F = spt_face(w, fn[2]); z = fma(F - Fprev, nrd, 0.0);
+        *reinterpret_cast<double2*>(Pp + 14) = make_double2(hold, z);
+    }
+}
+
+// z sweep that also writes the component out: the zone that a step completes gets A = P + z contribution and, fused,
+// U_next = U_m + ca A + sum c_r P_r straight from the sweep (a half warp covers 16 consecutive zones of a row: full
+// 128-byte segments), so the separate write-out phase of the next pass -- and its read of the partial-sum tile -- is gone.
+// Operands of the update are requested one group of four zones ahead.  Same operations in the same order as
+// spt_write_out: bit-identical results.
+struct SptOut {              // per-thread addresses of the zone column (i, j, k = 0 .. 15) of component c
+    const double* um; double* un; double* a; const double* p[UPD_MAX_EXT];
+    long long ustep, astep;
+};
+template <int NR>
+__device__ __forceinline__ void spt_sweep_z_out(const double* __restrict__ Xp, const double* __restrict__ Pp,
+                                                const double* __restrict__ fm, const double (&hx)[6], const double nrd,
+                                                const unsigned long long keep, const UpdArgs& up, SptOut o)
+{
+    constexpr int XS = SptDir<2>::XS, PS = SptDir<2>::PS;
+    const unsigned long long strm = spt_policy_stream();
+    PpmWindow w;
+    double fn[4], fnn[4];
+    const double f0 = spt_ldg(fm, keep), f1 = spt_ldg(fm + NTHR, keep);
+#pragma unroll
+    for (int e = 0; e < 4; ++e) fn[e] = spt_ldg(fm + (2 + e) * NTHR, keep);
+#pragma unroll
+    for (int e = 0; e < 4; ++e) fnn[e] = spt_ldg(fm + (6 + e) * NTHR, keep);
+    // operands of zone 0 and of the first group (zones 1 .. 4)
+    double um0 = 0.0, pv0[UPD_MAX_EXT] = {}, umn[4] = {}, pvn[4][UPD_MAX_EXT] = {};
+    if (NR >= 0) {
+        um0 = spt_ldg(o.um, strm);
+#pragma unroll
+        for (int r = 0; r < NR; ++r) pv0[r] = spt_ldg(o.p[r], strm);
+#pragma unroll
+        for (int e = 0; e < 4; ++e) {
+            umn[e] = spt_ldg(o.um + (1 + e) * o.ustep, strm);
+#pragma unroll
+            for (int r = 0; r < NR; ++r) pvn[e][r] = spt_ldg(o.p[r] + (1 + e) * o.astep, strm);
+        }
+    }
+    auto emit = [&](const int q, const double av, const double um, const double (&pv)[UPD_MAX_EXT]) {
+        if (NR >= 0) {
+            double acc = fma(up.ca, av, um);
+#pragma unroll
+            for (int r = 0; r < NR; ++r) acc = fma(up.c[r], pv[r], acc);
+            spt_stg(o.un + q * o.ustep, acc, strm);
+        }
+        spt_stg(o.a + q * o.astep, av, strm);
+    };
+    w.start(hx[0]); w.warm1(hx[1]); w.warm2(hx[2]);
+    w.warm3(Xp[0]);
+    w.push(Xp[XS]);
+    w.push(Xp[2 * XS]);
+    const double F0 = spt_face(w, f0);
+    w.push(Xp[3 * XS]);
+    double Fprev = spt_face(w, f1);
+    emit(0, fma(Fprev - F0, nrd, Pp[0]), um0, pv0);
+#pragma unroll 1
+    for (int it = 1; it <= 3; ++it) {                 // positions 4it .. 4it+3: faces 4it-2 .., zones 4it-3 .. 4it
+        double fc[4], umc[4] = {}, pvc[4][UPD_MAX_EXT] = {};
+#pragma unroll
+        for (int e = 0; e < 4; ++e) {
+            fc[e] = fn[e];
+            fn[e] = fnn[e];
+            if (it < 2 || (it == 2 && e < 3)) fnn[e] = spt_ldg(fm + (4 * it + 6 + e) * NTHR, keep);
+            if (NR >= 0) {
+                umc[e] = umn[e];
+#pragma unroll
+                for (int r = 0; r < NR; ++r) pvc[e][r] = pvn[e][r];
+                const int qn = 4 * it + 1 + e;                     // zone of the next group (13 .. 15 in the tail)
+                if (qn < TILE) {
+                    umn[e] = spt_ldg(o.um + qn * o.ustep, strm);
+#pragma unroll
+                    for (int r = 0; r < NR; ++r) pvn[e][r] = spt_ldg(o.p[r] + qn * o.astep, strm);
+                }
+            }
+        }
+        const double* __restrict__ xg = Xp + 4 * it * XS;
+        const double* __restrict__ pg = Pp + (4 * it - 3) * PS;
+#pragma unroll
+        for (int e = 0; e < 4; ++e) {
+            w.push(xg[e * XS]);
+            const double F = spt_face(w, fc[e]);
+            emit(4 * it - 3 + e, fma(F - Fprev, nrd, pg[e * PS]), umc[e], pvc[e]);
+            Fprev = F;
+        }
+    }
+#pragma unroll
+    for (int e = 0; e < 3; ++e) {
+        w.push(hx[3 + e]);
+        const double F = spt_face(w, fn[e]);
+        emit(13 + e, fma(F - Fprev, nrd, Pp[(13 + e) * PS]), umn[e], pvn[e]);
+        Fprev = F;
     }
 }
 
@@ -373,4 +536,93 @@ __device__ __forceinline__ void spt_tile(const Geom& g, const TileCoord& tc, con
         }
     }
     spt_write_out<NR>(g, tc, PB, A, up, 5 + s_end - 1);
+}
+
+// the species [s_begin, s_end) of one full tile, variant kernels: V = 1 forms X inside the x sweep (no conversion phase);
+// V = 2 also writes each component out from its own z sweep (no write-out phase, one barrier fewer per species; the tile
+// load of the next species is then issued right after the z sweep and is hidden only by the other CTA of the SM).
+template <int NR, int V>
+__device__ __forceinline__ void spt_tile_v(const Geom& g, const TileCoord& tc, const SptMaps& maps,
+                                           const double* __restrict__ Ub, const double* __restrict__ rinv_b,
+                                           const double* __restrict__ fm_tile, double* __restrict__ A, const UpdArgs& up,
+                                           double* __restrict__ sm, const int s_begin, const int s_end)
+{
+    constexpr bool ZOUT = (V == 2);
+    const int ng = CST_NG;
+    double* Xs = sm;                                  // [SPT_XTILE]
+    double* PB = sm + SPT_XTILE;                      // [SPT_TILE]
+    uint64_t* bar = reinterpret_cast<uint64_t*>(sm + SPT_XTILE + SPT_TILE);
+    const int tid = threadIdx.x, a = tid & (TILE - 1), b = tid >> 4;
+    const int tx = tc.i0 + ng - 4, ty = tc.j0 + ng;
+    const int zc0 = (tc.b * g.nvar) * g.ez + tc.k0 + ng;
+    const int za0 = (tc.b * g.nvar) * g.nz + tc.k0;
+    if (tid == 0) {
+        mbar_init(bar, 1);
+        fence_mbar_init();
+        mbar_expect_tx(bar, SPT_XTILE_BYTES);
+        tma_load_3d(Xs, &maps.u, tx, ty, zc0 + (5 + s_begin) * g.ez, bar);
+        bulk_prefetch_l2(fm_tile, 3 * (TILE + 1) * NTHR * 8);
+        tma_prefetch_3d(&maps.r, tc.i0, tc.j0 + 1, tc.b * g.ez + tc.k0 + 1);
+    }
+    __syncthreads();                                  // the initialised barrier is visible to every waiter
+    const double nrdx = -g.rdx, nrdy = -g.rdy, nrdz = -g.rdz;
+    const double* __restrict__ fm = fm_tile + tid;
+    // ghosted index of the tile origin; the x pencil (j = a, k = b) starts four zones to the left of it
+    const long long zt = ((long long)(tc.k0 + ng) * g.ey + (tc.j0 + ng)) * g.ex + (tc.i0 + ng);
+    const double* __restrict__ rrow = rinv_b + zt + (long long)b * g.plane_g + (long long)a * g.ex - 4;
+    // z pencil (i = a, j = b): the column of zones this thread completes
+    const long long ucol = (long long)tc.b * g.box_g + zt + (long long)b * g.ex + a;
+    const long long acol = (long long)tc.b * g.box_a + ((long long)tc.k0 * g.ny + tc.j0 + b) * g.nx + tc.i0 + a;
+    int n = 0;
+#pragma unroll 1
+    for (int s = s_begin; s < s_end; ++s, ++n) {
+        const int c = 5 + s;
+        const bool last = (s + 1 >= s_end);
+        const unsigned long long keep = last ? spt_policy_stream() : spt_policy_keep();
+        const double* Us = Ub + (long long)c * g.comp_g;
+        if (!ZOUT && n > 0) spt_write_out<NR>(g, tc, PB, A, up, c - 1);
+        if (tid == 0) {
+            if (!last) tma_prefetch_3d(&maps.u, tx, ty, zc0 + (c + 1) * g.ez);
+            if (NR > 0) {
+#pragma unroll
+                for (int r = 0; r < NR; ++r) tma_prefetch_3d(&maps.p[r], tc.i0, tc.j0, za0 + c * g.nz);
+            }
+        }
+        SptHalo hr;
+        spt_halo_load(g, tc, 1, Us, rinv_b, hr, keep);           // operands of the y sweep: in flight during the x sweep
+        if (!ZOUT && n > 0) __syncthreads();          // P free (written out); with ZOUT the barrier after the z sweep did that
+        mbar_wait(bar, n & 1);                        // the raw tile has landed (every thread reads only its own row next)
+        double hx[6];
+        // ---- x sweep (+ conversion)
+        spt_sweep_x_conv(Xs + spt_xbase<0>(a, b), PB + spt_pbase<0>(a, b), fm, rrow, nrdx, keep);
+        __syncthreads();
+        // ---- y sweep
+#pragma unroll
+        for (int m = 0; m < 6; ++m) hx[m] = hr.u[m] * hr.r[m];
+        spt_halo_load(g, tc, 2, Us, rinv_b, hr, keep);
+        spt_sweep_yz<1>(Xs + spt_xbase<1>(a, b), PB + spt_pbase<1>(a, b), fm + (TILE + 1) * NTHR, hx, nrdy, keep);
+        __syncthreads();
+        // ---- z sweep (+ write-out)
+#pragma unroll
+        for (int m = 0; m < 6; ++m) hx[m] = hr.u[m] * hr.r[m];
+        if (ZOUT) {
+            SptOut o;
+            o.ustep = g.plane_g; o.astep = (long long)g.ny * g.nx;
+            o.um = (NR >= 0) ? up.U_m + ucol + (long long)c * g.comp_g : nullptr;
+            o.un = (NR >= 0) ? up.U_next + ucol + (long long)c * g.comp_g : nullptr;
+            o.a = A + acol + (long long)c * g.comp_a;
+#pragma unroll
+            for (int r = 0; r < UPD_MAX_EXT; ++r) o.p[r] = (r < NR) ? up.P[r] + acol + (long long)c * g.comp_a : nullptr;
+            spt_sweep_z_out<NR>(Xs + spt_xbase<2>(a, b), PB + spt_pbase<2>(a, b), fm + 2 * (TILE + 1) * NTHR, hx, nrdz, keep, up, o);
+        } else {
+            spt_sweep_yz<2>(Xs + spt_xbase<2>(a, b), PB + spt_pbase<2>(a, b), fm + 2 * (TILE + 1) * NTHR, hx, nrdz, keep);
+        }
+        __syncthreads();                              // X released (and, with ZOUT, P read)
+        if (tid == 0 && !last) {
+            fence_proxy_async();
+            mbar_expect_tx(bar, SPT_XTILE_BYTES);
+            tma_load_3d(Xs, &maps.u, tx, ty, zc0 + (c + 1) * g.ez, bar);
+        }
+    }
+    if (!ZOUT) spt_write_out<NR>(g, tc, PB, A, up, 5 + s_end - 1);
 }

@@ -1,0 +1,86 @@
+"""The kernel variants of the species half of <A(U)> (include/cst.h cst_set_variant, cst_tune_advance): every variant
+against the oracle at the usual gate, bitwise against variant 0, for every fused-update arity, and the tuner."""
+import numpy as np
+import pytest
+import torch
+
+from oracle import orc
+from paper_1910_12578_b200 import Context, CstError, workloads as wl
+from test_oracle_pins import small_cfg
+
+pytestmark = pytest.mark.gpu
+TOL = 1e-12
+DEV = "cuda:0"
+
+
+def dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).to(DEV)
+
+
+def comp_err(gpu, ref):
+    axes = (0, 2, 3, 4)
+    num, den = np.abs(gpu - ref).max(axis=axes), np.abs(ref).max(axis=axes)
+    return np.where(den > 0, num / np.where(den > 0, den, 1.0), num)
+
+
+@pytest.mark.parametrize("n,nb,ns,bc", [
+    ((32, 16, 16), (1, 1, 1), 13, (0, 0, 0)),         # two tiles in x, the three-CTAs-per-tile split (5 / 4 / 4 species)
+    ((16, 32, 32), (2, 1, 1), 4, (1, 2, 0)),          # boxes, outflow / reflecting shells, gravity
+    ((16, 16, 16), (1, 1, 1), 1, (0, 0, 0)),          # one species: one CTA per tile, a single pass
+    ((16, 16, 48), (1, 1, 1), 2, (0, 0, 0)),          # split 2, one species per CTA
+])
+def test_variants_match_oracle_and_each_other(n, nb, ns, bc):
+    cfg = small_cfg(n=n, nb=nb, nspec=ns, gamma=5 / 3, bc=bc, grav=(0.0, 0.1, -0.2))
+    U = orc.fill_ghosts(cfg, wl.random_state(cfg, 111))
+    Ao = orc.advance_A(cfg, U)
+    dt = 0.4 * orc.cfl_dt(cfg, U, 0.5)
+    rng = np.random.default_rng(7)
+    P = [Ao + 0.1 * rng.standard_normal(Ao.shape) * np.abs(Ao).max() for _ in range(3)]
+    Ud, Pd = dev(U), [dev(p) for p in P]
+    ctx = Context(cfg)
+    with pytest.raises(CstError):
+        ctx.set_variant(3)
+    # update arities: plain A (NR = -1), forward Euler (0 external arrays), 1, 2, 3 external arrays
+    cases = {"plain": None, "nr0": ("self", []), "nr1": (0, [0]), "nr2": (0, [0, 1]), "nr3": (0, [1, 2])}
+    ref = {}
+    for v in (0, 1, 2):
+        ctx.set_variant(v)
+        assert ctx.get_variant() == v
+        for name, case in cases.items():
+            A = torch.full(wl.a_shape(cfg), float("nan"), dtype=torch.float64, device=DEV)
+            Un = torch.full(wl.u_shape(cfg), 3.0, dtype=torch.float64, device=DEV)
+            if case is None:
+                ctx.advance_A(Ud, A)
+            else:
+                old, quad = case
+                Aold = A if old == "self" else Pd[old]
+                Aq = [Pd[q] for q in quad] + [A]
+                w = [0.3 * dt / len(Aq)] * len(Aq)
+                ctx.advance_A_update(Ud, A, Un, dt, Aold, Aq, w)
+                Uno = np.full_like(U, 3.0)
+                orc.sdc_update(cfg, Uno, U, dt, Ao, Ao if old == "self" else P[old], [P[q] for q in quad] + [Ao], w)
+                assert comp_err(Un.cpu().numpy(), Uno).max() <= 10 * TOL, (v, name)
+            Ah = A.cpu().numpy()
+            assert comp_err(Ah, Ao).max() <= TOL, (v, name)
+            if v == 0:
+                ref[name] = (Ah, Un.cpu().numpy())
+            else:
+                assert np.array_equal(Ah, ref[name][0]) and np.array_equal(Un.cpu().numpy(), ref[name][1]), (v, name)
+    ctx.destroy()
+
+
+def test_tuner_keeps_a_valid_variant_and_valid_outputs():
+    cfg = small_cfg(n=(32, 16, 16), nspec=3, gamma=5 / 3)
+    U = orc.fill_ghosts(cfg, wl.random_state(cfg, 112))
+    Ao = orc.advance_A(cfg, U)
+    ctx = Context(cfg)
+    Ud = dev(U)
+    A = torch.full(wl.a_shape(cfg), float("nan"), dtype=torch.float64, device=DEV)
+    Un = torch.full(wl.u_shape(cfg), 3.0, dtype=torch.float64, device=DEV)
+    v, ms = ctx.tune_advance(Ud, A, Un, 1e-3, A, [A, A], [5e-4, 5e-4], repeats=1)
+    assert v in (0, 1, 2) and len(ms) == 3 and all(m > 0 for m in ms) and ms[v] == min(ms)
+    assert comp_err(A.cpu().numpy(), Ao).max() <= TOL
+    Uno = np.full_like(U, 3.0)
+    orc.sdc_update(cfg, Uno, U, 1e-3, Ao, Ao, [Ao, Ao], [5e-4, 5e-4])
+    assert comp_err(Un.cpu().numpy(), Uno).max() <= TOL
+    ctx.destroy()
