@@ -15,7 +15,8 @@ EXPORTS = ["cst_create", "cst_destroy", "cst_workspace_bytes", "cst_set_workspac
            "cst_advance_A_update", "cst_cfl_dt_device", "cst_cfl_dt", "cst_validate", "cst_step_host",
            "cst_set_timing", "cst_last_advance_ms", "cst_launch_count", "cst_strerror", "cst_version",
            "cst_debug_rcp_sqrt", "cst_debug_tile_count", "cst_debug_tile_map",
-           "cst_set_variant", "cst_get_variant", "cst_tune_advance", "cst_set_order", "cst_set_flattening", "cst_set_diffusion", "cst_set_reactions", "cst_react_R", "cst_sdc_update_react", "cst_react_failures",
+           "cst_set_variant", "cst_get_variant", "cst_set_species_split", "cst_get_species_split",
+           "cst_tune_advance", "cst_set_order", "cst_set_flattening", "cst_set_diffusion", "cst_set_reactions", "cst_react_R", "cst_sdc_update_react", "cst_react_failures",
            "cst_exchange_plan", "cst_set_sublattice", "cst_exchange_info", "cst_exchange_pack", "cst_exchange_unpack"]
 
 
@@ -87,6 +88,8 @@ def load():
     lib.cst_launch_count.restype = C.c_longlong
     lib.cst_set_variant.argtypes = [_vp, C.c_int]
     lib.cst_get_variant.argtypes = [_vp]
+    lib.cst_set_species_split.argtypes = [_vp, C.c_int]
+    lib.cst_get_species_split.argtypes = [_vp]
     lib.cst_tune_advance.argtypes = [_vp, _vp, _vp, _vp, C.c_double, _vp, C.c_int, C.POINTER(_vp), _dp, C.c_int,
                                      C.POINTER(C.c_float), _vp]
     lib.cst_set_order.argtypes = [_vp, C.c_int]
@@ -247,11 +250,17 @@ class Context:
     def get_variant(self):
         return int(self.lib.cst_get_variant(self._h))
 
+    def set_species_split(self, split):
+        self._check(self.lib.cst_set_species_split(self._h, int(split)), "cst_set_species_split")
+
+    def get_species_split(self):
+        return int(self.lib.cst_get_species_split(self._h))
+
     def tune_advance(self, U_m, A_new_m, U_next, dt_m, A_old_m, A_quad, w_quad, repeats=2, stream=None):
         """cst_tune_advance: times the fused advance with every species-kernel variant, keeps the fastest.
-        -> (chosen variant, [ms of variant 0, 1, 2])."""
+        -> (chosen variant, [ms of variant 0, 1, 2 at the default split, ms of the winner at split 2 and 4])."""
         n, arr, w = self._quad(A_quad, w_quad)
-        ms = (C.c_float * 3)()
+        ms = (C.c_float * 5)()
         self._check(self.lib.cst_tune_advance(self._h, _ptr(U_m), _ptr(A_new_m), _ptr(U_next), float(dt_m), _ptr(A_old_m),
                                               n, arr, w, int(repeats), ms, _stream(stream)), "cst_tune_advance")
         return self.get_variant(), [float(x) for x in ms]

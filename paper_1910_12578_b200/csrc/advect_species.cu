@@ -194,7 +194,8 @@ static int launch_species_nr(cst_ctx* ctx, const double* U, double* A, const Upd
     if (tma) {
         if (cudaFuncSetAttribute(k_advect_species_tma<NR>, cudaFuncAttributeMaxDynamicSharedMemorySize, SPT_SMEM) != cudaSuccess)
             return CST_ECUDA;
-        const int split = g.nspec < SPT_SPLIT ? g.nspec : SPT_SPLIT;
+        const int want = ctx->species_split > 0 ? ctx->species_split : SPT_SPLIT;
+        const int split = g.nspec < want ? g.nspec : want;
         const unsigned grid = (unsigned)(tg.ntiles * split);
         if (ctx->species_variant == 1) {
             if (cudaFuncSetAttribute(k_advect_species_tma_v<NR, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, SPT_SMEM) != cudaSuccess)

@@ -69,6 +69,7 @@ extern "C" int cst_create(const cst_params* p, cst_ctx** out)
     c->flatten = 0;
     c->order = 2;
     c->species_variant = 0;
+    c->species_split = 0;
     for (int n = 0; n < 3; ++n) c->ev[n] = nullptr;
     int dev = 0;
     cudaError_t e = cudaGetDevice(&dev);
@@ -223,7 +224,15 @@ extern "C" int cst_set_variant(cst_ctx* c, int species_variant)
     return CST_OK;
 }
 
+extern "C" int cst_set_species_split(cst_ctx* c, int split)
+{
+    if (!c || split < 0 || split > 8) return CST_EINVAL;
+    c->species_split = split;
+    return CST_OK;
+}
+
 extern "C" int cst_get_variant(const cst_ctx* c) { return c ? c->species_variant : CST_EINVAL; }
+extern "C" int cst_get_species_split(const cst_ctx* c) { return c ? c->species_split : CST_EINVAL; }
 
 // Times the fused advance with every species-kernel variant on the caller's own buffers and keeps the fastest.
 extern "C" int cst_tune_advance(cst_ctx* c, const double* U_m, double* A_new_m, double* U_next, double dt_m,
@@ -257,10 +266,29 @@ extern "C" int cst_tune_advance(cst_ctx* c, const double* U_m, double* A_new_m, 
         if (ms_out) ms_out[v] = ms_v;
         if (v == 0 || ms_v < best_ms) { best = v; best_ms = ms_v; }
     }
+    c->species_variant = (rc == CST_OK) ? best : 0;
+    // second knob, for the winner only: how many CTAs share one tile (default 3); keep another value only if it is faster
+    int best_split = 0;
+    for (int sp = 2; sp <= 4 && rc == CST_OK; sp += 2) {
+        c->species_split = sp;
+        float ms_s = 0.f;
+        for (int n = 0; n <= repeats && rc == CST_OK; ++n) {
+            cudaEventRecord(e0, st);
+            rc = cst_advance_A_update(c, U_m, A_new_m, U_next, dt_m, A_old_m, nquad, A_quad, w_quad, stream);
+            cudaEventRecord(e1, st);
+            if (rc != CST_OK) break;
+            if (cudaEventSynchronize(e1) != cudaSuccess) { rc = cuda_fail(cudaGetLastError()); break; }
+            float ms = 0.f;
+            cudaEventElapsedTime(&ms, e0, e1);
+            if (n == 1 || (n > 1 && ms < ms_s)) ms_s = ms;
+        }
+        if (ms_out) ms_out[3 + (sp == 4)] = ms_s;
+        if (rc == CST_OK && ms_s < best_ms) { best_split = sp; best_ms = ms_s; }
+    }
+    c->species_split = (rc == CST_OK) ? best_split : 0;
     cudaEventDestroy(e0); cudaEventDestroy(e1);
     c->timing = keep_timing;
-    c->species_variant = (rc == CST_OK) ? best : 0;
-    if (rc == CST_OK && best != 2)      // leave the outputs as the chosen kernel writes them (all variants agree bit for bit)
+    if (rc == CST_OK)                   // leave the outputs as the chosen configuration writes them (all agree bit for bit)
         rc = cst_advance_A_update(c, U_m, A_new_m, U_next, dt_m, A_old_m, nquad, A_quad, w_quad, stream);
     return rc;
 }

@@ -40,6 +40,7 @@ struct cst_ctx {
     struct XPlan* xplan;     // cst_set_sublattice: ghost-exchange plan with the neighbouring ranks (exchange.cu)
     cst_react_params react;  // cst_set_reactions (react.cu)
     int has_react;
+    int species_split;       // CTAs that share one tile in the species kernel (each a contiguous share of the species); 0 = default
     int species_variant;     // cst_set_variant / cst_tune_advance: 0 measured kernel, 1 / 2 variant kernels (species_tma.cuh)
     int order;               // cst_set_order: 2 (PPM path, default) or 4 (fourth.cu)
     int flatten;             // cst_set_flattening (flatten.cu): chi array behind rinv and Fm in the workspace

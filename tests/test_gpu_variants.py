@@ -66,6 +66,13 @@ def test_variants_match_oracle_and_each_other(n, nb, ns, bc):
                 ref[name] = (Ah, Un.cpu().numpy())
             else:
                 assert np.array_equal(Ah, ref[name][0]) and np.array_equal(Un.cpu().numpy(), ref[name][1]), (v, name)
+    # the number of CTAs that share a tile does not change a bit either
+    ctx.set_variant(2)
+    for split in (1, 2, 4, 8):
+        ctx.set_species_split(split)
+        A = torch.full(wl.a_shape(cfg), float("nan"), dtype=torch.float64, device=DEV)
+        ctx.advance_A(Ud, A)
+        assert np.array_equal(A.cpu().numpy(), ref["plain"][0]), split
     ctx.destroy()
 
 
@@ -78,7 +85,10 @@ def test_tuner_keeps_a_valid_variant_and_valid_outputs():
     A = torch.full(wl.a_shape(cfg), float("nan"), dtype=torch.float64, device=DEV)
     Un = torch.full(wl.u_shape(cfg), 3.0, dtype=torch.float64, device=DEV)
     v, ms = ctx.tune_advance(Ud, A, Un, 1e-3, A, [A, A], [5e-4, 5e-4], repeats=1)
-    assert v in (0, 1, 2) and len(ms) == 3 and all(m > 0 for m in ms) and ms[v] == min(ms)
+    assert v in (0, 1, 2) and len(ms) == 5 and all(m > 0 for m in ms) and ms[v] == min(ms[:3])
+    assert ctx.get_species_split() in (0, 2, 4)
+    if ctx.get_species_split():
+        assert ms[3 + (ctx.get_species_split() == 4)] == min(ms)
     assert comp_err(A.cpu().numpy(), Ao).max() <= TOL
     Uno = np.full_like(U, 3.0)
     orc.sdc_update(cfg, Uno, U, 1e-3, Ao, Ao, [Ao, Ao], [5e-4, 5e-4])
