@@ -43,6 +43,7 @@ def lib():
         _lib.orc_advance_A.argtypes = [P, _dp, _dp]
         _lib.orc_advance_A_flat.argtypes = [P, _dp, _dp]
         _lib.orc_advance_A4.argtypes = [P, _dp, _dp]
+        _lib.orc_advance_ctu.argtypes = [P, _dp, C.c_double, _dp]
         _lib.orc_ppm4_line.argtypes = [C.c_int, _dp, _dp, _dp]
         _lib.orc_ppm4_line.restype = None
         _lib.orc_flatten_line.argtypes = [C.c_int, _dp, _dp, C.c_double, _dp]
@@ -138,6 +139,25 @@ def advance_A4(cfg, U, A=None):
         A = np.empty(a_shape(cfg), dtype=np.float64)
     _chk(lib().orc_advance_A4(C.byref(make_params(cfg)), _ptr(U), _ptr(A)), "advance_A4")
     return A
+
+
+def advance_ctu(cfg, U, dt, A=None):
+    """A_ctu(U, dt) = -div F^{n+1/2} + S of the unsplit CTU PPM scheme (oracle/orc_ctu.c, readings C1-C9);
+    U^{n+1} = U^n + dt A_ctu.  The whole ghost shell must be filled."""
+    assert U.shape == u_shape(cfg)
+    if A is None:
+        A = np.empty(a_shape(cfg), dtype=np.float64)
+    _chk(lib().orc_advance_ctu(C.byref(make_params(cfg)), _ptr(U), float(dt), _ptr(A)), "advance_ctu")
+    return A
+
+
+def ctu_step(cfg, U, dt):
+    """One CTU step from library calls of the oracle: ghost fill, A_ctu, U + dt A_ctu.  Returns the new ghosted state."""
+    U0 = fill_ghosts(cfg, U.copy())
+    A = advance_ctu(cfg, U0, dt)
+    Un = U0.copy()
+    sdc_update(cfg, Un, U0, dt, A, A, [A], [dt])          # U + dt (A - A) + dt A
+    return Un
 
 
 def ppm4_line(q):
