@@ -148,6 +148,17 @@ int cst_tune_advance(cst_ctx* ctx, const double* U_m, double* A_new_m, double* U
                      const double* A_old_m, int nquad, const double* const* A_quad, const double* w_quad,
                      int repeats, float* ms_out, void* stream);
 
+/* The unsplit CTU PPM operator ("the main unsplit PPM hydrodynamics scheme [15, 16]", the hydro solver of the
+ * paper's Strang path; readings C1-C9): PPM parabolas with characteristic tracing over
+ * dt / 2 (Colella & Woodward 1984), corner-transport-upwind transverse flux corrections (Miller & Colella 2002: one third
+ * of dt for the first, one half for the final states; 12 HLLC solves per zone), divergence + gravity source:
+ *   A <- A_ctu(U, dt) = -div F^{n+1/2} + S,      U^{n+1} = U^n + dt A   (e.g. cst_sdc_update with A_new = A_old, w = dt).
+ * Unlike <A(U)> of the SDC path it depends on dt and is stable for dt <= min_d Delta_d / max(|u_d| + c).  Reads the
+ * WHOLE 4-deep ghost shell.  workspace_dev: DEVICE scratch of cst_ctu_workspace_bytes() bytes (18 arrays of the size of
+ * U), 16-byte aligned, owned by the caller (CST_ENOWORKSPACE if too small).  CST_EINVAL: NULL, dt < 0. */
+long long cst_ctu_workspace_bytes(const cst_ctx* ctx);
+int cst_advance_ctu(cst_ctx* ctx, const double* U, double dt, double* A, void* workspace_dev, long long bytes, void* stream);
+
 /* Spatial order of <A(U)> ("a fourth-order method in space and time (using a Simpsons rule for the integral and
  * the spatial reconstruction of [12])"; readings G1-G9).  order = 2 (default, the graded
  * path): PPM + CW84 limiter as described at cst_advance_A.  order = 4: U and A are CELL AVERAGES and every later

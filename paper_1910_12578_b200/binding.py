@@ -16,7 +16,7 @@ EXPORTS = ["cst_create", "cst_destroy", "cst_workspace_bytes", "cst_set_workspac
            "cst_set_timing", "cst_last_advance_ms", "cst_launch_count", "cst_strerror", "cst_version",
            "cst_debug_rcp_sqrt", "cst_debug_tile_count", "cst_debug_tile_map",
            "cst_set_variant", "cst_get_variant", "cst_set_species_split", "cst_get_species_split",
-           "cst_tune_advance", "cst_set_order", "cst_set_flattening", "cst_set_diffusion", "cst_set_reactions", "cst_react_R", "cst_sdc_update_react", "cst_react_failures",
+           "cst_tune_advance", "cst_ctu_workspace_bytes", "cst_advance_ctu", "cst_set_order", "cst_set_flattening", "cst_set_diffusion", "cst_set_reactions", "cst_react_R", "cst_sdc_update_react", "cst_react_failures",
            "cst_exchange_plan", "cst_set_sublattice", "cst_exchange_info", "cst_exchange_pack", "cst_exchange_unpack"]
 
 
@@ -92,6 +92,9 @@ def load():
     lib.cst_get_species_split.argtypes = [_vp]
     lib.cst_tune_advance.argtypes = [_vp, _vp, _vp, _vp, C.c_double, _vp, C.c_int, C.POINTER(_vp), _dp, C.c_int,
                                      C.POINTER(C.c_float), _vp]
+    lib.cst_ctu_workspace_bytes.argtypes = [_vp]
+    lib.cst_ctu_workspace_bytes.restype = C.c_longlong
+    lib.cst_advance_ctu.argtypes = [_vp, _vp, C.c_double, _vp, _vp, C.c_longlong, _vp]
     lib.cst_set_order.argtypes = [_vp, C.c_int]
     lib.cst_set_flattening.argtypes = [_vp, C.c_int]
     lib.cst_set_diffusion.argtypes = [_vp, C.c_double, C.c_double]
@@ -264,6 +267,15 @@ class Context:
         self._check(self.lib.cst_tune_advance(self._h, _ptr(U_m), _ptr(A_new_m), _ptr(U_next), float(dt_m), _ptr(A_old_m),
                                               n, arr, w, int(repeats), ms, _stream(stream)), "cst_tune_advance")
         return self.get_variant(), [float(x) for x in ms]
+
+    def ctu_workspace_bytes(self):
+        return int(self.lib.cst_ctu_workspace_bytes(self._h))
+
+    def advance_ctu(self, U, dt, A, workspace, stream=None):
+        """A <- A_ctu(U, dt) (unsplit CTU PPM); workspace: contiguous device tensor of >= ctu_workspace_bytes() bytes."""
+        nbytes = workspace.numel() * workspace.element_size()
+        self._check(self.lib.cst_advance_ctu(self._h, _ptr(U), float(dt), _ptr(A), workspace.data_ptr(), nbytes,
+                                             _stream(stream)), "cst_advance_ctu")
 
     def set_order(self, order):
         """Spatial order of <A(U)>: 2 (default) or 4; changes workspace_bytes(): set the workspace afterwards."""

@@ -293,6 +293,19 @@ extern "C" int cst_tune_advance(cst_ctx* c, const double* U_m, double* A_new_m, 
     return rc;
 }
 
+extern "C" long long cst_ctu_workspace_bytes(const cst_ctx* c)
+{
+    return c ? ctu_workspace_doubles(c->g) * (long long)sizeof(double) : -1;
+}
+
+extern "C" int cst_advance_ctu(cst_ctx* c, const double* U, double dt, double* A, void* workspace_dev, long long bytes,
+                               void* stream)
+{
+    if (!c || !U || !A || !workspace_dev || !(dt >= 0.0)) return CST_EINVAL;
+    if (bytes < cst_ctu_workspace_bytes(c) || ((uintptr_t)workspace_dev & 15)) return CST_ENOWORKSPACE;
+    return check_launch(launch_advance_ctu(c, U, dt, A, (double*)workspace_dev, (cudaStream_t)stream));
+}
+
 extern "C" int cst_set_order(cst_ctx* c, int order)
 {
     if (!c || (order != 2 && order != 4)) return CST_EINVAL;

@@ -76,6 +76,8 @@ int launch_cfl(cst_ctx*, const double* U, double cfl, double* dt_out_dev, cudaSt
 int launch_validate(cst_ctx*, const double* U, cudaStream_t);   // count left in d_scratch[2]
 int launch_advance_A4(cst_ctx*, const double* U, double* A, cudaStream_t);   // fourth.cu: fourth-order <A(U)>
 long long fourth_workspace_doubles(const Geom& g);
+int launch_advance_ctu(cst_ctx*, const double* U, double dt, double* A, double* ws, cudaStream_t);   // ctu.cu
+long long ctu_workspace_doubles(const Geom& g);
 int launch_flatten(cst_ctx*, const double* U, cudaStream_t);   // flatten.cu: chi of every zone -1 .. n -> workspace
 // diffuse.cu: A[rho E] += k_th lap T (and U_next[rho E] += ca * that when U_next != nullptr)
 int launch_diffuse_add(cst_ctx*, const double* U, double* A, double* U_next, double ca, cudaStream_t);
