@@ -244,7 +244,8 @@ int cst_validate(cst_ctx* ctx, const double* U, long long* n_bad_host, void* str
 /* Host-buffer convenience used for the end-to-end measurement: copies the interior+ghost array
  * U_host (HOST, layout of U) to the device buffers owned by the caller (U_dev, U_next_dev,
  * A_dev), runs fill_ghosts + advance_A_update (forward-Euler node update: A_old = A_quad = A_new)
- * and copies A and U_next back to A_host / U_next_host.  Synchronises the stream. */
+ * and copies A and U_next back to A_host / U_next_host.  As with every node update only interior zones of U_next are
+ * written: the ghost zones of U_next_host are whatever U_next_dev held before the call.  Synchronises the stream. */
 int cst_step_host(cst_ctx* ctx, const double* U_host, double* A_host, double* U_next_host,
                   double* U_dev, double* U_next_dev, double* A_dev,
                   double dt_m, void* stream);   /* needs the workspace, see cst_set_workspace */

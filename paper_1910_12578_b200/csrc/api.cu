@@ -202,9 +202,7 @@ extern "C" int cst_step_host(cst_ctx* c, const double* U_host, double* A_host, d
     const size_t ub = (size_t)g.box_g * g.nbox * sizeof(double), ab = (size_t)g.box_a * g.nbox * sizeof(double);
     cudaError_t e = cudaMemcpyAsync(U_dev, U_host, ub, cudaMemcpyHostToDevice, st);
     if (e != cudaSuccess) return cuda_fail(e);
-    // U_next starts as a copy of U_m so that its ghost shell is defined (stale, as documented)
-    e = cudaMemcpyAsync(U_next_dev, U_dev, ub, cudaMemcpyDeviceToDevice, st);
-    if (e != cudaSuccess) return cuda_fail(e);
+    // only interior zones of U_next are written: its ghost shell keeps whatever U_next_dev held (cst.h)
     int rc = check_launch(launch_fill_ghosts(c, U_dev, st));
     if (rc) return rc;
     QuadArgs q{};
