@@ -46,6 +46,8 @@ def parse():
                     help="time this config only (default: configs[3], then configs[4] under \"also\")")
     ap.add_argument("--n", type=int, default=None, help="override zones per box side (debug only; marks the line)")
     ap.add_argument("--no-tune", action="store_true", help="keep species-kernel variant 0 instead of timing the variants")
+    ap.add_argument("--exchange", default="sendrecv", choices=["sendrecv", "p2p"],
+                    help="multi-GPU ghost exchange: NCCL send/recv of packed messages, or direct stores into peer-mapped memory")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     return ap.parse_args()
@@ -265,7 +267,10 @@ def measure(cfg, args, rank, world, local, dev, want_e2e, want_cpu_baseline):
     dt_dev = torch.zeros(1, dtype=torch.float64, device=dev)
     ex = None
     if world > 1:                 # ghost zones with a source on another rank travel through NCCL send/recv
-        ex = shard.GhostExchange(ctx, gcfg, part, rank, lambda n: torch.empty(n, dtype=torch.float64, device=dev))
+        mode = getattr(args, "exchange", "sendrecv")
+        ex = shard.GhostExchange(ctx, gcfg, part, rank, lambda n: torch.empty(n, dtype=torch.float64, device=dev), mode=mode)
+        if mode == "p2p":
+            ex.register(U)          # IPC handles of U to the peers; raises if the allocation cannot be shared
     fill = (lambda: ex.fill_ghosts(U)) if ex else (lambda: ctx.fill_ghosts(U))
     fill()
     dt = ctx.cfl_dt(U, 0.5)
@@ -441,8 +446,9 @@ def measure(cfg, args, rank, world, local, dev, want_e2e, want_cpu_baseline):
                                        f"{gcfg['nx']}x{gcfg['ny']}x{gcfg['nz']}+{gcfg['ng']} ghosts, NVAR={N}",
                            "zones_per_gpu": zones, "zones_total": zones * world,
                            "step": "fill_ghosts + advance_A_update + cfl_dt_device" if ex is None else
-                                   "fill_ghosts + exchange_pack + NCCL send/recv + exchange_unpack + advance_A_update + "
-                                   "cfl_dt_device + all_reduce(MIN) of dt",
+                                   ("fill_ghosts + exchange_pack + NCCL send/recv + exchange_unpack" if ex.mode == "sendrecv" else
+                                    "barrier + fill_ghosts + exchange_push (stores into peer-mapped memory) + barrier")
+                                   + " + advance_A_update + cfl_dt_device + all_reduce(MIN) of dt",
                            "ghost_exchange_bytes_per_rank_per_step": ex.bytes_per_fill if ex else 0,
                            "l2": f"inputs larger than L2 ({(ubytes + 3 * abytes) / 1e9:.1f} GB touched per step)"
                                  if ubytes > 4e8 else "inputs fit in L2 (debug size)",

@@ -102,7 +102,10 @@ typedef struct {
     int ext[3];            /* zones per direction (extents of the destination region)                        */
     int flip[3];           /* send: 1 = the momentum component along d changes sign (reflecting wall)        */
     long long offset;      /* doubles from the start of this peer's message; segment data is [c][k][j][i]    */
+    int rbox;              /* the OTHER side's local box index (recv: the source box there; send: the box whose */
+    int rlo[3];            /* ghost region is filled) and the first zone of the segment there                  */
 } cst_xseg;
+#define CST_MAX_PEERS 26
 long long cst_exchange_plan(const cst_params* global, const int part[3], int rank, int recv,
                             cst_xseg* segs, long long cap);
 int cst_set_sublattice(cst_ctx* ctx, const int global_nb[3], const int part[3], int rank);
@@ -110,6 +113,21 @@ int cst_exchange_info(const cst_ctx* ctx, int* npeers, int* peers, long long* se
                       long long* recv_off, long long* recv_len, int cap);
 int cst_exchange_pack(cst_ctx* ctx, const double* U, double* sendbuf, void* stream);
 int cst_exchange_unpack(cst_ctx* ctx, double* U, const double* recvbuf, void* stream);
+
+/* The same exchange without staging buffers or a communication library: cst_exchange_push writes every zone that a
+ * peer's ghost shell reads from this brick STRAIGHT into the peer's state array through a peer-mapped device pointer
+ * (stores over NVLink / NVSwitch from one kernel; same zone map and signs as pack + unpack).  peer_U: HOST array of
+ * npeers DEVICE pointers, in the order of cst_exchange_info, each the base of that peer's U (its whole brick).  The
+ * caller separates pushes from the peers' reads of their shells (a barrier across the ranks before the push and one
+ * after it, e.g. torch.distributed.barrier).
+ * Pointers to another process's memory come from CUDA IPC: cst_ipc_export gives a 64-byte handle of the allocation
+ * that contains dev_ptr plus the offset of dev_ptr inside it; cst_ipc_import opens such a handle in another process
+ * and returns the mapped pointer (+ offset); cst_ipc_close unmaps it (pass the pointer minus the offset).
+ * CST_ECUDA if the allocation cannot be shared (peer access unavailable, or an allocator that does not use cudaMalloc). */
+int cst_exchange_push(cst_ctx* ctx, const double* U, double* const* peer_U, int npeers, void* stream);
+int cst_ipc_export(const void* dev_ptr, unsigned char handle[64], long long* offset_bytes);
+int cst_ipc_import(const unsigned char handle[64], long long offset_bytes, void** dev_ptr);
+int cst_ipc_close(void* mapped_base);
 
 /* S1-S4.  A <- <A(U)>: conserved->primitive with the gamma-law EOS, PPM
  * reconstruction (Colella & Woodward 1984 limiter, P:L52 ref [15]) of the primitives in x, y, z,

@@ -17,7 +17,8 @@ EXPORTS = ["cst_create", "cst_destroy", "cst_workspace_bytes", "cst_set_workspac
            "cst_debug_rcp_sqrt", "cst_debug_tile_count", "cst_debug_tile_map",
            "cst_set_variant", "cst_get_variant", "cst_set_species_split", "cst_get_species_split",
            "cst_tune_advance", "cst_ctu_workspace_bytes", "cst_advance_ctu", "cst_set_order", "cst_set_flattening", "cst_set_diffusion", "cst_set_reactions", "cst_react_R", "cst_sdc_update_react", "cst_react_failures",
-           "cst_exchange_plan", "cst_set_sublattice", "cst_exchange_info", "cst_exchange_pack", "cst_exchange_unpack"]
+           "cst_exchange_plan", "cst_set_sublattice", "cst_exchange_info", "cst_exchange_pack", "cst_exchange_unpack",
+           "cst_exchange_push", "cst_ipc_export", "cst_ipc_import", "cst_ipc_close"]
 
 
 class CstParams(C.Structure):
@@ -42,7 +43,8 @@ class CstReactParams(C.Structure):
 class CstXseg(C.Structure):
     """cst_xseg of include/cst.h: one ghost region that crosses ranks."""
     _fields_ = [("peer", C.c_int), ("box", C.c_int), ("lo", C.c_int * 3), ("step", C.c_int * 3),
-                ("ext", C.c_int * 3), ("flip", C.c_int * 3), ("offset", C.c_longlong)]
+                ("ext", C.c_int * 3), ("flip", C.c_int * 3), ("offset", C.c_longlong),
+                ("rbox", C.c_int), ("rlo", C.c_int * 3)]
 
 
 class CstError(RuntimeError):
@@ -110,6 +112,10 @@ def load():
     lib.cst_exchange_info.argtypes = [_vp, I3, I3, LLP, LLP, LLP, LLP, C.c_int]
     lib.cst_exchange_pack.argtypes = [_vp, _vp, _vp, _vp]
     lib.cst_exchange_unpack.argtypes = [_vp, _vp, _vp, _vp]
+    lib.cst_exchange_push.argtypes = [_vp, _vp, C.POINTER(_vp), C.c_int, _vp]
+    lib.cst_ipc_export.argtypes = [_vp, C.c_char_p, LLP]
+    lib.cst_ipc_import.argtypes = [C.c_char_p, C.c_longlong, C.POINTER(_vp)]
+    lib.cst_ipc_close.argtypes = [_vp]
     lib.cst_strerror.argtypes = [C.c_int]
     lib.cst_strerror.restype = C.c_char_p
     lib.cst_version.restype = C.c_char_p
@@ -142,6 +148,31 @@ def exchange_plan(cfg_global, part, rank, recv):
     segs = (CstXseg * max(int(n), 1))()
     lib.cst_exchange_plan(C.byref(p), pa, int(rank), int(bool(recv)), segs, n)
     return [segs[i] for i in range(int(n))]
+
+
+def ipc_export(t):
+    """(64-byte handle, offset) of the CUDA allocation that holds the tensor / address t, for cst_ipc_import elsewhere."""
+    lib = load()
+    h = C.create_string_buffer(64)
+    off = C.c_longlong(0)
+    rc = lib.cst_ipc_export(_ptr(t), h, C.byref(off))
+    if rc:
+        raise CstError(rc, "cst_ipc_export", lib.cst_strerror(rc).decode())
+    return h.raw, off.value
+
+
+def ipc_import(handle, offset):
+    """device address (int) of another process's array; close with ipc_close(address - offset)."""
+    lib = load()
+    p = _vp()
+    rc = lib.cst_ipc_import(handle, int(offset), C.byref(p))
+    if rc:
+        raise CstError(rc, "cst_ipc_import", lib.cst_strerror(rc).decode())
+    return int(p.value)
+
+
+def ipc_close(mapped_base):
+    load().cst_ipc_close(int(mapped_base))
 
 
 def _ptr(t):
@@ -336,6 +367,12 @@ class Context:
 
     def exchange_unpack(self, U, recvbuf, stream=None):
         self._check(self.lib.cst_exchange_unpack(self._h, _ptr(U), _ptr(recvbuf), _stream(stream)), "cst_exchange_unpack")
+
+    def exchange_push(self, U, peer_U, stream=None):
+        """peer_U: one device array / address per peer (exchange_info order): the base of that peer's U."""
+        n = len(peer_U)
+        arr = (_vp * max(n, 1))(*[_ptr(p) for p in peer_U])
+        self._check(self.lib.cst_exchange_push(self._h, _ptr(U), arr, n, _stream(stream)), "cst_exchange_push")
 
     def set_timing(self, on):
         self._check(self.lib.cst_set_timing(self._h, int(bool(on))), "cst_set_timing")

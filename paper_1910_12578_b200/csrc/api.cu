@@ -398,6 +398,54 @@ extern "C" int cst_exchange_unpack(cst_ctx* c, double* U, const double* recvbuf,
     return check_launch(launch_exchange_unpack(c, U, recvbuf, (cudaStream_t)stream));
 }
 
+extern "C" int cst_exchange_push(cst_ctx* c, const double* U, double* const* peer_U, int npeers, void* stream)
+{
+    if (!c || !U || (npeers > 0 && !peer_U) || npeers < 0) return CST_EINVAL;
+    return check_launch(launch_exchange_push(c, U, peer_U, npeers, (cudaStream_t)stream));
+}
+
+// CUDA IPC: share the allocation that contains dev_ptr with another process (the ghost exchange over peer memory)
+extern "C" int cst_ipc_export(const void* dev_ptr, unsigned char handle[64], long long* offset_bytes)
+{
+    if (!dev_ptr || !handle || !offset_bytes) return CST_EINVAL;
+    static_assert(sizeof(cudaIpcMemHandle_t) == 64, "IPC handle size");
+    // base of the allocation: the driver's cuMemGetAddressRange (libcst does not link libcuda)
+    typedef int (*range_fn)(unsigned long long*, size_t*, unsigned long long);
+    void* fp = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuMemGetAddressRange", &fp, cudaEnableDefault, &q) != cudaSuccess ||
+        q != cudaDriverEntryPointSuccess || !fp)
+        return cuda_fail(cudaGetLastError());
+    unsigned long long base = 0;
+    size_t size = 0;
+    if (((range_fn)fp)(&base, &size, (unsigned long long)(uintptr_t)dev_ptr) != 0) return CST_EINVAL;
+    cudaIpcMemHandle_t h;
+    const cudaError_t e = cudaIpcGetMemHandle(&h, (void*)(uintptr_t)base);
+    if (e != cudaSuccess) return cuda_fail(e);
+    memcpy(handle, &h, 64);
+    *offset_bytes = (long long)((unsigned long long)(uintptr_t)dev_ptr - base);
+    return CST_OK;
+}
+
+extern "C" int cst_ipc_import(const unsigned char handle[64], long long offset_bytes, void** dev_ptr)
+{
+    if (!handle || !dev_ptr || offset_bytes < 0) return CST_EINVAL;
+    cudaIpcMemHandle_t h;
+    memcpy(&h, handle, 64);
+    void* base = nullptr;
+    const cudaError_t e = cudaIpcOpenMemHandle(&base, h, cudaIpcMemLazyEnablePeerAccess);
+    if (e != cudaSuccess) return cuda_fail(e);
+    *dev_ptr = (char*)base + offset_bytes;
+    return CST_OK;
+}
+
+extern "C" int cst_ipc_close(void* mapped_base)
+{
+    if (!mapped_base) return CST_EINVAL;
+    const cudaError_t e = cudaIpcCloseMemHandle(mapped_base);
+    return e == cudaSuccess ? CST_OK : cuda_fail(e);
+}
+
 extern "C" int cst_set_timing(cst_ctx* c, int on)
 {
     if (!c) return CST_EINVAL;

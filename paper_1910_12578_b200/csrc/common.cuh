@@ -93,6 +93,7 @@ int xplan_info(const cst_ctx*, int* npeers, int* peers, long long* send_off, lon
                long long* recv_off, long long* recv_len, int cap);
 int launch_exchange_pack(cst_ctx*, const double* U, double* sendbuf, cudaStream_t);
 int launch_exchange_unpack(cst_ctx*, double* U, const double* recvbuf, cudaStream_t);
+int launch_exchange_push(cst_ctx*, const double* U, double* const* peer_U, int npeers, cudaStream_t);
 int launch_debug_rcp_sqrt(const double* x, double* r, double* s, long long n, cudaStream_t);
 long long debug_tile_count(const Geom& g);
 int launch_debug_tile_map(cst_ctx*, int* out, cudaStream_t);

@@ -145,8 +145,8 @@ void plan_segments(const Lattice& L, int rank, int recv, std::vector<cst_xseg>& 
             for (const RawSeg& s : raw) {
                 if (s.src_rank != q) continue;
                 cst_xseg x;
-                x.peer = q; x.box = s.dst_box; x.offset = off;
-                for (int d = 0; d < 3; ++d) { x.lo[d] = s.dlo[d]; x.step[d] = 1; x.ext[d] = s.ext[d]; x.flip[d] = 0; }
+                x.peer = q; x.box = s.dst_box; x.offset = off; x.rbox = s.src_box;
+                for (int d = 0; d < 3; ++d) { x.lo[d] = s.dlo[d]; x.step[d] = 1; x.ext[d] = s.ext[d]; x.flip[d] = 0; x.rlo[d] = s.slo[d]; }
                 off += (long long)L.nvar * s.ext[0] * s.ext[1] * s.ext[2];
                 out.push_back(x);
             }
@@ -159,8 +159,8 @@ void plan_segments(const Lattice& L, int rank, int recv, std::vector<cst_xseg>& 
             for (const RawSeg& s : raw) {
                 if (s.src_rank != rank) continue;
                 cst_xseg x;
-                x.peer = q; x.box = s.src_box; x.offset = off;
-                for (int d = 0; d < 3; ++d) { x.lo[d] = s.slo[d]; x.step[d] = s.step[d]; x.ext[d] = s.ext[d]; x.flip[d] = s.flip[d]; }
+                x.peer = q; x.box = s.src_box; x.offset = off; x.rbox = s.dst_box;
+                for (int d = 0; d < 3; ++d) { x.lo[d] = s.slo[d]; x.step[d] = s.step[d]; x.ext[d] = s.ext[d]; x.flip[d] = s.flip[d]; x.rlo[d] = s.dlo[d]; }
                 off += (long long)L.nvar * s.ext[0] * s.ext[1] * s.ext[2];
                 out.push_back(x);
             }
@@ -171,6 +171,7 @@ void plan_segments(const Lattice& L, int rank, int recv, std::vector<cst_xseg>& 
 struct DevSeg {
     int box;
     int lo[3], step[3], ext[3], flip[3];
+    int peer_slot, rbox, rlo[3];   // send segments: index of the peer in the plan's peer list, destination box / first zone there
     long long off;            // doubles from the start of the whole send / receive buffer
     long long zone_start;     // first zone (all components) of this segment in the flat thread index
 };
@@ -207,6 +208,8 @@ static long long upload(const std::vector<cst_xseg>& v, const std::vector<int>& 
         for (int d = 0; d < 3; ++d) { s.lo[d] = v[n].lo[d]; s.step[d] = v[n].step[d]; s.ext[d] = v[n].ext[d]; s.flip[d] = v[n].flip[d]; }
         const size_t pi = std::lower_bound(peers.begin(), peers.end(), v[n].peer) - peers.begin();
         s.off = base[pi] + v[n].offset;
+        s.peer_slot = (int)pi; s.rbox = v[n].rbox;
+        for (int d = 0; d < 3; ++d) s.rlo[d] = v[n].rlo[d];
         s.zone_start = z;
         z += (long long)s.ext[0] * s.ext[1] * s.ext[2];
     }
@@ -320,6 +323,50 @@ k_exchange(Geom g, const DevSeg* __restrict__ segs, int nseg, long long zones, d
             }
         }
     }
+}
+
+// The exchange WITHOUT staging buffers: every zone a peer's ghost shell reads from this brick is written straight into
+// the peer's array through a peer-mapped pointer (NVLink stores; the caller obtained the pointers with cst_ipc_import
+// or, in one process, passes the arrays themselves).  Same zone map and signs as pack + unpack.
+struct PeerPtrs { double* p[CST_MAX_PEERS]; };
+__global__ void __launch_bounds__(256)
+k_exchange_push(Geom g, const DevSeg* __restrict__ segs, int nseg, long long zones, const double* __restrict__ U, PeerPtrs peers)
+{
+    for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < zones; t += (long long)gridDim.x * blockDim.x) {
+        int lo = 0, hi = nseg - 1;
+        while (lo < hi) {
+            const int mid = (lo + hi + 1) >> 1;
+            if (segs[mid].zone_start <= t) lo = mid; else hi = mid - 1;
+        }
+        const DevSeg& s = segs[lo];
+        const long long z = t - s.zone_start;
+        const int ix = (int)(z % s.ext[0]);
+        const long long r = z / s.ext[0];
+        const int iy = (int)(r % s.ext[1]), iz = (int)(r / s.ext[1]);
+        const long long u0 = uidx(g, s.box, 0, s.lo[2] + s.step[2] * iz, s.lo[1] + s.step[1] * iy, s.lo[0] + s.step[0] * ix);
+        const long long d0 = uidx(g, s.rbox, 0, s.rlo[2] + iz, s.rlo[1] + iy, s.rlo[0] + ix);     // every brick has the same shape
+        double* __restrict__ dst = peers.p[s.peer_slot] + d0;
+        for (int c = 0; c < g.nvar; ++c) {
+            const double v = U[u0 + c * g.comp_g];
+            const bool neg = (c >= 1 && c <= 3) && s.flip[c - 1];
+            dst[c * g.comp_g] = neg ? -v : v;
+        }
+    }
+}
+
+int launch_exchange_push(cst_ctx* ctx, const double* U, double* const* peer_U, int npeers, cudaStream_t st)
+{
+    const XPlan* xp = ctx->xplan;
+    if (!xp || npeers != (int)xp->peers.size() || npeers > CST_MAX_PEERS) return CST_EINVAL;
+    if (xp->zones_send == 0) return CST_OK;
+    PeerPtrs pp{};
+    for (int n = 0; n < npeers; ++n) { if (!peer_U[n]) return CST_EINVAL; pp.p[n] = peer_U[n]; }
+    long long nb = (xp->zones_send + 255) / 256;
+    const long long cap = (long long)ctx->sm_count * 16;
+    if (nb > cap) nb = cap;
+    k_exchange_push<<<(unsigned)nb, 256, 0, st>>>(ctx->g, xp->d_send, (int)xp->n_send, xp->zones_send, U, pp);
+    ctx->launches++;
+    return cudaGetLastError() == cudaSuccess ? CST_OK : CST_ECUDA;
 }
 
 static int launch_exchange(cst_ctx* ctx, double* U, double* buf, bool pack, cudaStream_t st)

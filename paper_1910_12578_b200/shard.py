@@ -54,23 +54,64 @@ def local_boxes(cfg_global, part, rank):
 
 
 class GhostExchange:
-    """Ghost fill of a sharded lattice: local fill + pack + point-to-point messages + unpack.
+    """Ghost fill of a sharded lattice.  Two transports:
+
+    mode="sendrecv" (default): local fill + cst_exchange_pack + one torch.distributed point-to-point message per peer
+        + cst_exchange_unpack (NCCL send/recv on GPUs, gloo in the CPU tests);
+    mode="p2p": local fill + cst_exchange_push -- ONE kernel that stores every zone the peers' shells read from this
+        brick straight into the peers' arrays through peer-mapped pointers (CUDA IPC over NVLink / NVSwitch), no staging
+        buffers, no communication library on the data path; two barriers separate the pushes from the peers' reads.
+        Every state array that is ghost-filled must be registered once (register(U)): its IPC handle goes to the peers.
 
     ctx: binding.Context of the rank's brick (local_config) -- set_sublattice is called here.
     alloc(n_doubles) -> a float64 buffer on the device of U (torch tensor)."""
 
-    def __init__(self, ctx, cfg_global, part, rank, alloc):
-        self.ctx, self.rank = ctx, rank
+    def __init__(self, ctx, cfg_global, part, rank, alloc, mode="sendrecv"):
+        self.ctx, self.rank, self.mode = ctx, rank, mode
         ctx.set_sublattice((cfg_global["nbx"], cfg_global["nby"], cfg_global["nbz"]), part, rank)
         self.info = ctx.exchange_info()
         ns = sum(i[2] for i in self.info)
         nr = sum(i[4] for i in self.info)
-        self.sendbuf, self.recvbuf = alloc(max(ns, 1)), alloc(max(nr, 1))
         self.bytes_per_fill = 8 * (ns + nr)
+        self._peer_ptrs = {}                    # data_ptr of a registered U -> the peers' mapped addresses
+        self._mapped = []
+        if mode == "sendrecv":
+            self.sendbuf, self.recvbuf = alloc(max(ns, 1)), alloc(max(nr, 1))
+        elif mode != "p2p":
+            raise ValueError("mode must be 'sendrecv' or 'p2p'")
+
+    def register(self, U):
+        """p2p: make U reachable by the peers and map their corresponding arrays (collective: every rank calls it with
+        its own array, in the same order)."""
+        import torch.distributed as dist
+        from . import binding
+        handle, off = binding.ipc_export(U)
+        everyone = [None] * dist.get_world_size()
+        dist.all_gather_object(everyone, (handle, off))
+        ptrs = []
+        for peer, *_ in self.info:
+            addr = binding.ipc_import(*everyone[peer])
+            self._mapped.append(addr - everyone[peer][1])
+            ptrs.append(addr)
+        self._peer_ptrs[U.data_ptr()] = ptrs
+
+    def close(self):
+        from . import binding
+        for base in self._mapped:
+            binding.ipc_close(base)
+        self._mapped, self._peer_ptrs = [], {}
 
     def fill_ghosts(self, U, stream=None):
         """Complete ghost fill of the local boxes of U (in place)."""
         import torch.distributed as dist
+        if self.mode == "p2p" and self.info:
+            import torch
+            dist.barrier()                      # the peers have finished reading the shells this push overwrites
+            self.ctx.fill_ghosts(U, stream)
+            self.ctx.exchange_push(U, self._peer_ptrs[U.data_ptr()], stream)
+            torch.cuda.synchronize()            # my stores have landed ...
+            dist.barrier()                      # ... and so have everyone else's
+            return
         self.ctx.fill_ghosts(U, stream)
         if not self.info:
             return

@@ -86,6 +86,38 @@ def test_sharded_lattice_equals_single_lattice_bitwise(n, gnb, bc, part, nspec):
     ctx1.destroy()
 
 
+@pytest.mark.parametrize("n,gnb,bc,part", [
+    ((8, 6, 5), (2, 2, 2), (0, 0, 0), (2, 2, 2)),
+    ((6, 4, 4), (4, 2, 1), (0, 1, 2), (2, 2, 1)),
+    ((4, 4, 7), (2, 3, 4), (2, 0, 1), (1, 3, 2)),
+])
+def test_push_exchange_through_peer_pointers_equals_global_fill(n, gnb, bc, part):
+    """cst_exchange_push: every rank stores straight into the other ranks' arrays (here all in one process, so the
+    "peer-mapped" pointers are the arrays themselves); no buffers, no unpack."""
+    cfg = small_cfg(n=n, nb=gnb, nspec=2, bc=bc)
+    U_host = wl.random_state(cfg, 42)
+    Uo = orc.fill_ghosts(cfg, U_host.copy())
+    world = part[0] * part[1] * part[2]
+    lc = shard.local_config(cfg, part)
+    ranks = []
+    for r in range(world):
+        ctx = Context(lc)
+        ctx.set_sublattice((cfg["nbx"], cfg["nby"], cfg["nbz"]), part, r)
+        ranks.append(dict(ctx=ctx, U=dev(U_host[shard.local_boxes(cfg, part, r)])))
+    for me in ranks:
+        me["ctx"].fill_ghosts(me["U"])
+    torch.cuda.synchronize()
+    for me in ranks:
+        peers = [ranks[i[0]]["U"] for i in me["ctx"].exchange_info()]
+        me["ctx"].exchange_push(me["U"], peers)
+    torch.cuda.synchronize()
+    for r, me in enumerate(ranks):
+        assert np.array_equal(me["U"].cpu().numpy(), Uo[shard.local_boxes(cfg, part, r)]), f"rank {r}"
+        with pytest.raises(CstError):
+            me["ctx"].exchange_push(me["U"], [])                 # wrong number of peers
+        me["ctx"].destroy()
+
+
 def test_sublattice_errors():
     cfg = small_cfg(n=(4, 4, 4), nb=(2, 1, 1))
     ctx = Context(cfg)
