@@ -281,7 +281,7 @@ def measure(cfg, args, rank, world, local, dev, want_e2e, want_cpu_baseline):
     w = [0.5 * dt, 0.5 * dt]
 
     # kernel variants of the species half (cst_tune_advance): every variant is timed on these buffers before the
-    # warm-up steps and the fastest is kept; all variants give bit-identical results (tests/test_gpu_variants.py)
+    # warm-up steps and the fastest is kept; all variants give bit-identical results (tests/test_next_gpu_variants.py)
     tuned = {"species_variant": 0, "ms": None, "note": "not tuned"}
     if not getattr(args, "no_tune", False) and N > 5:
         try:

@@ -1,7 +1,7 @@
 """The N > 1 path of bench.py on CPU: world_size 2, gloo.  The box lattice is sharded over the ranks (DESIGN.md
 section 9): the scalar reductions (MIN of dt, MAX of the device time), the sharded workload and each rank's share of
 the seeded input are checked here; the ghost exchange itself in tests/test_shard_plan.py (gloo) and
-tests/test_gpu_shard.py (kernels)."""
+tests/test_next_gpu_shard.py (kernels)."""
 import os
 import sys
 

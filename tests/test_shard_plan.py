@@ -153,7 +153,7 @@ def test_brick_partition():
 # ------------------------------------------------------------------ world size 2, gloo: the message plumbing ----
 class NumpyBrickCtx:
     """Stand-in for binding.Context in the CPU test: the same five calls GhostExchange makes, executed with numpy
-    from the library's host-side plan (the CUDA pack / unpack kernels are covered by tests/test_gpu_shard.py)."""
+    from the library's host-side plan (the CUDA pack / unpack kernels are covered by tests/test_next_gpu_shard.py)."""
 
     def __init__(self, cfg_global, local_filled):
         self.cfg, self.local_filled = cfg_global, local_filled
