@@ -157,7 +157,7 @@ def oracle_sample_cfg(cfg):
     else:
         n = min(cfg["nx"], 144)
         c = wl.make_config(cfg["index"], n=n, nspec=cfg["nspec"])
-        what = f"same input distribution on a {n}^3 box (1 of {max(1, (cfg['nx'] // n) ** 3)} sub-volumes)"
+        what = f"same input distribution on a {n}^3 box ({n ** 3 / (cfg['nx'] * cfg['ny'] * cfg['nz']):.3f} of the zones)"
     return c, what
 
 
@@ -188,7 +188,7 @@ def run_reference(args, cfg, rank):
     cb, sec = time_oracle(cfg, steps, warmup)
     line = {"impl": "reference", "metric": METRIC, "value": cb["value"], "unit": UNIT, "n_gpus": args.gpus,
             "steps": steps, "warmup": warmup, "ms_per_step": sec * 1e3, "higher_is_better": True,
-            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "scaling": "strong", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": f"configs[{cfg['index']}] {cfg['name']} (bounded sample: {cb['sample']})"},
             "cpu_baseline": cb,
             "e2e": {"value": cb["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
