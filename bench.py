@@ -298,6 +298,7 @@ def measure(cfg, args, rank, world, local, dev, want_e2e, want_cpu_baseline):
     ctx.set_timing(True)      # CUDA events around the two kernels of the advance, on this stream (cst.h)
 
     step_ev = []
+    fused_cfl = {"on": False, "ms_separate": None, "ms_fused": None}
 
     def step(timed):
         if timed:
@@ -306,11 +307,15 @@ def measure(cfg, args, rank, world, local, dev, want_e2e, want_cpu_baseline):
         if timed:
             e0, e1 = ev(), ev()
             e0.record()
-        ctx.advance_A_update(U, A_new, U_next, dt, A_old0, [A_old0, A_old1], w)
+        if fused_cfl["on"]:       # S1-S6 in one call: the CFL max is gathered inside the hydro kernel's z sweep
+            ctx.advance_A_update_cfl(U, A_new, U_next, dt, A_old0, [A_old0, A_old1], w, 0.5, dt_dev)
+        else:
+            ctx.advance_A_update(U, A_new, U_next, dt, A_old0, [A_old0, A_old1], w)
         if timed:
             e1.record()
             k_ev.append((e0, e1))
-        ctx.cfl_dt_device(U, 0.5, dt_dev)
+        if not fused_cfl["on"]:
+            ctx.cfl_dt_device(U, 0.5, dt_dev)
         if world > 1:
             dist.all_reduce(dt_dev, op=dist.ReduceOp.MIN)
 
@@ -319,6 +324,28 @@ def measure(cfg, args, rank, world, local, dev, want_e2e, want_cpu_baseline):
             dist.barrier()
         torch.cuda.synchronize()
 
+    if not getattr(args, "no_tune", False):
+        # the step with the CFL reduction folded into the advance against the step with the separate CFL pass: 3 runs each
+        # after one untimed run, the faster composition is kept (same results: tests/test_next_gpu_variants.py)
+        try:
+            for key, on in (("ms_separate", False), ("ms_fused", True)):
+                fused_cfl["on"] = on
+                step(False)
+                torch.cuda.synchronize()
+                t0e, t1e = ev(), ev()
+                t0e.record()
+                for _ in range(3):
+                    step(False)
+                t1e.record()
+                torch.cuda.synchronize()
+                fused_cfl[key] = t0e.elapsed_time(t1e) / 3
+            fused_cfl["on"] = fused_cfl["ms_fused"] < fused_cfl["ms_separate"]
+        except Exception as exc:
+            fused_cfl.update(on=False, note=f"comparison failed ({exc})")
+        if world > 1:             # every rank must run the same composition: all take rank 0's choice
+            flag = torch.tensor([1.0 if fused_cfl["on"] else 0.0], dtype=torch.float64, device=dev)
+            dist.broadcast(flag, 0)
+            fused_cfl["on"] = bool(flag.item() > 0.5)
     for _ in range(args.warmup):
         step(False)
     sync_all()
@@ -445,7 +472,8 @@ def measure(cfg, args, rank, world, local, dev, want_e2e, want_cpu_baseline):
                 "config": {"workload": f"configs[{gcfg['index']}] {gcfg['name']}: {gcfg['nbx'] * gcfg['nby'] * gcfg['nbz']} box(es) of "
                                        f"{gcfg['nx']}x{gcfg['ny']}x{gcfg['nz']}+{gcfg['ng']} ghosts, NVAR={N}",
                            "zones_per_gpu": zones, "zones_total": zones * world,
-                           "step": "fill_ghosts + advance_A_update + cfl_dt_device" if ex is None else
+                           "step": ("fill_ghosts + advance_A_update_cfl" if fused_cfl["on"] else
+                                    "fill_ghosts + advance_A_update + cfl_dt_device") if ex is None else
                                    ("fill_ghosts + exchange_pack + NCCL send/recv + exchange_unpack" if ex.mode == "sendrecv" else
                                     "barrier + fill_ghosts + exchange_push (stores into peer-mapped memory) + barrier")
                                    + " + advance_A_update + cfl_dt_device + all_reduce(MIN) of dt",
@@ -455,7 +483,7 @@ def measure(cfg, args, rank, world, local, dev, want_e2e, want_cpu_baseline):
                            "parallelism": f"box lattice sharded over {world} ranks, bricks {part[0]}x{part[1]}x{part[2]}" if world > 1
                                           else "single GPU",
                            "ms_per_step_best": float(min(per_step)), "ms_per_step_median": float(np.median(per_step)),
-                           "tuned": tuned, "debug_size_override": bool(args.n)},
+                           "tuned": tuned, "fused_cfl": fused_cfl, "debug_size_override": bool(args.n)},
                 "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline,
                 "cpu_baseline": cpu_baseline}
     ctx.destroy()

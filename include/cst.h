@@ -247,6 +247,15 @@ int cst_advance_A_update(cst_ctx* ctx, const double* U_m, double* A_new_m, doubl
                          double dt_m, const double* A_old_m,
                          int nquad, const double* const* A_quad, const double* w_quad, void* stream);
 
+/* Fused S1-S6: cst_advance_A_update (same arguments, same rules) plus the CFL step of the SAME state U_m, left in
+ * *dt_out_dev (DEVICE pointer) as by cst_cfl_dt_device(ctx, U_m, cfl, ...).  On lattices made of full 16^3 tiles the max
+ * signal rate is gathered inside the z sweep of the hydro kernel, which has every zone's primitives at hand, and the
+ * separate pass over the state is saved; otherwise the two calls simply run back to back.  Does not synchronise. */
+int cst_advance_A_update_cfl(cst_ctx* ctx, const double* U_m, double* A_new_m, double* U_next,
+                             double dt_m, const double* A_old_m,
+                             int nquad, const double* const* A_quad, const double* w_quad,
+                             double cfl, double* dt_out_dev, void* stream);
+
 /* S6 (BASELINE.json north_star; sum form, Q20).
  *   dt = cfl / max over interior zones of [(|u|+c)/dx + (|v|+c)/dy + (|w|+c)/dz], c = sqrt(gamma p/rho)
  * cst_cfl_dt_device leaves dt in *dt_out_dev (DEVICE pointer) without synchronising;

@@ -12,7 +12,7 @@ LIB_PATH = os.environ.get("CST_LIB_PATH") or os.path.join(_HERE, "libcst.so")   
 MAX_QUAD = 4
 
 EXPORTS = ["cst_create", "cst_destroy", "cst_workspace_bytes", "cst_set_workspace", "cst_fill_ghosts", "cst_advance_A", "cst_sdc_update",
-           "cst_advance_A_update", "cst_cfl_dt_device", "cst_cfl_dt", "cst_validate", "cst_step_host",
+           "cst_advance_A_update", "cst_advance_A_update_cfl", "cst_cfl_dt_device", "cst_cfl_dt", "cst_validate", "cst_step_host",
            "cst_set_timing", "cst_last_advance_ms", "cst_launch_count", "cst_strerror", "cst_version",
            "cst_debug_rcp_sqrt", "cst_debug_tile_count", "cst_debug_tile_map",
            "cst_set_variant", "cst_get_variant", "cst_set_species_split", "cst_get_species_split",
@@ -76,6 +76,8 @@ def load():
     lib.cst_advance_A.argtypes = [_vp, _vp, _vp, _vp]
     lib.cst_sdc_update.argtypes = [_vp, _vp, _vp, C.c_double, _vp, _vp, C.c_int, C.POINTER(_vp), _dp, _vp]
     lib.cst_advance_A_update.argtypes = [_vp, _vp, _vp, _vp, C.c_double, _vp, C.c_int, C.POINTER(_vp), _dp, _vp]
+    lib.cst_advance_A_update_cfl.argtypes = [_vp, _vp, _vp, _vp, C.c_double, _vp, C.c_int, C.POINTER(_vp), _dp,
+                                             C.c_double, _vp, _vp]
     lib.cst_cfl_dt_device.argtypes = [_vp, _vp, C.c_double, _vp, _vp]
     lib.cst_cfl_dt.argtypes = [_vp, _vp, C.c_double, _dp, _vp]
     lib.cst_validate.argtypes = [_vp, _vp, C.POINTER(C.c_longlong), _vp]
@@ -258,6 +260,12 @@ class Context:
         self._check(self.lib.cst_advance_A_update(self._h, _ptr(U_m), _ptr(A_new_m), _ptr(U_next), float(dt_m),
                                                   _ptr(A_old_m), n, arr, w, _stream(stream)),
                     "cst_advance_A_update")
+
+    def advance_A_update_cfl(self, U_m, A_new_m, U_next, dt_m, A_old_m, A_quad, w_quad, cfl, dt_out_dev, stream=None):
+        n, arr, w = self._quad(A_quad, w_quad)
+        self._check(self.lib.cst_advance_A_update_cfl(self._h, _ptr(U_m), _ptr(A_new_m), _ptr(U_next), float(dt_m),
+                                                      _ptr(A_old_m), n, arr, w, float(cfl), _ptr(dt_out_dev),
+                                                      _stream(stream)), "cst_advance_A_update_cfl")
 
     def cfl_dt_device(self, U, cfl, dt_out_dev, stream=None):
         self._check(self.lib.cst_cfl_dt_device(self._h, _ptr(U), float(cfl), _ptr(dt_out_dev), _stream(stream)),

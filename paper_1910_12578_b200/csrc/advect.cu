@@ -33,7 +33,7 @@ static bool make_upd(UpdArgs& up, const double* U, double* A, double* U_next, do
 }
 
 int launch_advance_A(cst_ctx* ctx, const double* U, double* A, double* U_next, double dt_m,
-                     const double* A_old_m, const QuadArgs& q, bool fused, cudaStream_t st)
+                     const double* A_old_m, const QuadArgs& q, bool fused, cudaStream_t st, double* cfl_scratch)
 {
     if (!ctx->ws || ctx->ws_bytes < workspace_bytes(ctx)) return CST_ENOWORKSPACE;
     UpdArgs up{};
@@ -49,7 +49,7 @@ int launch_advance_A(cst_ctx* ctx, const double* U, double* A, double* U_next, d
     }
     if (ctx->flatten && (rc = launch_flatten(ctx, U, st)) != CST_OK) return rc;
     if (ctx->timing) cudaEventRecord(ctx->ev[0], st);
-    rc = launch_advect_hydro(ctx, U, A, up, st);
+    rc = cfl_scratch ? launch_advect_hydro_cfl(ctx, U, A, up, cfl_scratch, st) : launch_advect_hydro(ctx, U, A, up, st);
     if (rc) return rc;
     if (ctx->timing) cudaEventRecord(ctx->ev[1], st);
     rc = launch_advect_species(ctx, U, A, up, st);
@@ -59,4 +59,21 @@ int launch_advance_A(cst_ctx* ctx, const double* U, double* A, double* U_next, d
     if (rc || !split) return rc;
     // too many distinct arrays for the fused epilogue: A first, then the plain update kernel
     return launch_sdc_update(ctx, U_next, U, dt_m, A, A_old_m, q, st);
+}
+
+// S1-S6 in one call: the advance above and the CFL step of the SAME state.  On lattices of full tiles (second-order
+// path) the max signal rate is gathered inside the hydro kernel's z sweep, which has every zone's primitives at hand --
+// the separate pass over the five hydro components (k_cfl_max) is then not needed; otherwise it runs after the advance.
+int launch_advance_A_cfl(cst_ctx* ctx, const double* U, double* A, double* U_next, double dt_m, const double* A_old_m,
+                         const QuadArgs& q, bool fused, double cfl, double* dt_out_dev, cudaStream_t st)
+{
+    if (ctx->order == 2 && hydro_cfl_eligible(ctx, U)) {
+        int rc = launch_cfl_reset(ctx, st);
+        if (!rc) rc = launch_advance_A(ctx, U, A, U_next, dt_m, A_old_m, q, fused, st, ctx->d_scratch);
+        if (!rc) rc = launch_cfl_final(ctx, cfl, dt_out_dev, st);
+        return rc;
+    }
+    int rc = launch_advance_A(ctx, U, A, U_next, dt_m, A_old_m, q, fused, st);
+    if (!rc) rc = launch_cfl(ctx, U, cfl, dt_out_dev, st);
+    return rc;
 }

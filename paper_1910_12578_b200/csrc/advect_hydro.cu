@@ -46,9 +46,10 @@ struct HydroMarch {           // per-thread state of one pencil march
     double* part;             // shared-memory partial of the zone that completes next (component 0)
     double* pA;               // z sweep: A of the zone that completes next (component 0)
     long long zc;             // z sweep: ghosted index (within the box) of that zone
+    double cfl;               // CFL = true: running max of the signal rate of the interior zones (S6)
 };
 
-template <int D, int NR>
+template <int D, int NR, bool CFL = false>
 __device__ __forceinline__ void hydro_zone(const Geom& g, const TileCoord& tc, HydroMarch& m, const int p,
                                            const double Uc[5], const double* __restrict__ Ub,
                                            double* __restrict__ rinv_b, const UpdArgs& up,
@@ -78,6 +79,11 @@ __device__ __forceinline__ void hydro_zone(const Geom& g, const TileCoord& tc, H
     const double r = cons_to_prim(g, Uc[0], Uc[1], Uc[2], Uc[3], Uc[4], W);
     if ((D == 2 && p >= 0 && p < L) || (p < 0 && ghost_lo) || (p >= L && ghost_hi))
         rinv_b[z0 + (long long)p * stride] = r;
+    if (CFL && D == 2 && p >= 0 && p < L) {             // S6 folded into the z sweep: the primitives of the zone are at hand
+        const double cs = sqrt_fast(g.gamma * W[4] * r);
+        const double rate = (fabs(W[1]) + cs) * g.rdx + (fabs(W[2]) + cs) * g.rdy + (fabs(W[3]) + cs) * g.rdz;
+        m.cfl = dmax(m.cfl, rate);
+    }
 #pragma unroll
     for (int c = 0; c < 5; ++c) m.w[c].push(W[c]);
     if (p >= 2) {
@@ -128,11 +134,11 @@ __device__ __forceinline__ void hydro_zone(const Geom& g, const TileCoord& tc, H
     }
 }
 
-template <int D, int NR>
-__device__ __forceinline__ void hydro_sweep_full(const Geom& g, const TileCoord& tc, const double* __restrict__ Ub,
-                                                 double* __restrict__ part, double* __restrict__ fm_tile,
-                                                 double* __restrict__ rinv_b, double* __restrict__ A,
-                                                 const UpdArgs& up)
+template <int D, int NR, bool CFL = false>
+__device__ __forceinline__ double hydro_sweep_full(const Geom& g, const TileCoord& tc, const double* __restrict__ Ub,
+                                                   double* __restrict__ part, double* __restrict__ fm_tile,
+                                                   double* __restrict__ rinv_b, double* __restrict__ A,
+                                                   const UpdArgs& up)
 {
     const int ng = CST_NG;
     constexpr int L = TILE;
@@ -156,6 +162,7 @@ __device__ __forceinline__ void hydro_sweep_full(const Geom& g, const TileCoord&
         m.w[c].q1 = m.w[c].q2 = m.w[c].dq1 = m.w[c].s2 = m.w[c].e = m.w[c].qp = 0.0;
         m.Fprev[c] = 0.0;
     }
+    m.cfl = 0.0;
     m.fm_slot = fm_tile + (D * (TILE + 1)) * NTHR + tid;
     m.part = part + sp0;
     m.pA = A + (long long)tc.b * g.box_a + ((long long)tc.k0 * g.ny + (tc.j0 + b)) * g.nx + (tc.i0 + a);
@@ -177,7 +184,7 @@ __device__ __forceinline__ void hydro_sweep_full(const Geom& g, const TileCoord&
                 const int p = 4 * G + e;
                 if ((e == 0 && G == -1) || (e == 3 && G == 4)) continue;
                 const double Uc[5] = { cur[0][e], cur[1][e], cur[2][e], cur[3][e], cur[4][e] };
-                hydro_zone<D, NR>(g, tc, m, p, Uc, Ub, rinv_b, up, z0, stride, ghost_lo, ghost_hi);
+                hydro_zone<D, NR, CFL>(g, tc, m, p, Uc, Ub, rinv_b, up, z0, stride, ghost_lo, ghost_hi);
             }
 #pragma unroll
             for (int c = 0; c < 5; ++c)
@@ -203,7 +210,7 @@ __device__ __forceinline__ void hydro_sweep_full(const Geom& g, const TileCoord&
 #pragma unroll
             for (int e = 0; e < 2; ++e) {
                 const double Uc[5] = { cur[0][e], cur[1][e], cur[2][e], cur[3][e], cur[4][e] };
-                hydro_zone<D, NR>(g, tc, m, p0 + e, Uc, Ub, rinv_b, up, z0, stride, ghost_lo, ghost_hi);
+                hydro_zone<D, NR, CFL>(g, tc, m, p0 + e, Uc, Ub, rinv_b, up, z0, stride, ghost_lo, ghost_hi);
             }
 #pragma unroll
             for (int c = 0; c < 5; ++c)
@@ -211,6 +218,7 @@ __device__ __forceinline__ void hydro_sweep_full(const Geom& g, const TileCoord&
                 for (int e = 0; e < 2; ++e) cur[c][e] = nxt[c][e];
         }
     }
+    return m.cfl;
 }
 
 // --------------------------------------------------------------------------- any tile extent ----
@@ -369,6 +377,70 @@ k_advect_hydro(Geom g, TileGeom tg, const double* __restrict__ U, double* __rest
         __syncthreads();
         hydro_sweep<2, NR, FLAT>(g, tc, Ub, part, fm_tile, rinv_b, A, up, chi_b);
     }
+}
+
+// <A(U)> (+ node update) of the hydro components with the CFL reduction of the SAME state folded into the z sweep
+// (include/cst.h cst_advance_A_update_cfl): only for lattices made of full tiles; the max signal rate of the CTA's zones
+// goes through warp shuffles and one atomicMax on the bit pattern of the non-negative double, as in cfl.cu.
+template <int NR>
+__global__ void __launch_bounds__(NTHR, 1)
+k_advect_hydro_cfl(Geom g, TileGeom tg, const double* __restrict__ U, double* __restrict__ A,
+                   double* __restrict__ rinv, double* __restrict__ Fm, UpdArgs up, double* __restrict__ cfl_scratch)
+{
+    extern __shared__ double part[];
+    __shared__ double wmax[NTHR / 32];
+    const TileCoord tc = tile_coord(g, tg, blockIdx.x);
+    const double* Ub = U + (long long)tc.b * g.box_g;
+    double* rinv_b = rinv + (long long)tc.b * g.comp_g;
+    double* fm_tile = Fm + tc.tile * 3LL * (TILE + 1) * NTHR;
+    hydro_sweep_full<0, NR>(g, tc, Ub, part, fm_tile, rinv_b, A, up);
+    __syncthreads();
+    hydro_sweep_full<1, NR>(g, tc, Ub, part, fm_tile, rinv_b, A, up);
+    __syncthreads();
+    double smax = hydro_sweep_full<2, NR, true>(g, tc, Ub, part, fm_tile, rinv_b, A, up);
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) smax = fmax(smax, __shfl_xor_sync(0xffffffffu, smax, o));
+    if ((threadIdx.x & 31) == 0) wmax[threadIdx.x >> 5] = smax;
+    __syncthreads();
+    if (threadIdx.x < 32) {
+        double m = threadIdx.x < NTHR / 32 ? wmax[threadIdx.x] : 0.0;
+#pragma unroll
+        for (int o = 4; o > 0; o >>= 1) m = fmax(m, __shfl_xor_sync(0xffffffffu, m, o));
+        if (threadIdx.x == 0)
+            atomicMax(reinterpret_cast<unsigned long long*>(cfl_scratch), (unsigned long long)__double_as_longlong(m));
+    }
+}
+
+template <int NR>
+static int launch_hydro_cfl_nr(cst_ctx* ctx, const double* U, double* A, const UpdArgs& up, double* cfl_scratch, cudaStream_t st)
+{
+    const Geom& g = ctx->g;
+    const TileGeom tg = make_tile_geom(g);
+    const size_t smem = 5ull * PART_COMP * sizeof(double);
+    if (cudaFuncSetAttribute(k_advect_hydro_cfl<NR>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
+        return CST_ECUDA;
+    k_advect_hydro_cfl<NR><<<(unsigned)tg.ntiles, NTHR, smem, st>>>(g, tg, U, A, ctx->ws, ctx->ws + ws_rinv_doubles(g), up, cfl_scratch);
+    ctx->launches++;
+    return cudaGetLastError() == cudaSuccess ? CST_OK : CST_ECUDA;
+}
+
+// true when the fused kernel can serve this call: every tile full, 32-byte aligned rows, no flattening
+bool hydro_cfl_eligible(const cst_ctx* ctx, const double* U)
+{
+    const Geom& g = ctx->g;
+    return !ctx->flatten && (g.nx % TILE == 0) && (g.ny % TILE == 0) && (g.nz % TILE == 0) && (((uintptr_t)U & 31) == 0);
+}
+
+int launch_advect_hydro_cfl(cst_ctx* ctx, const double* U, double* A, const UpdArgs& up, double* cfl_scratch, cudaStream_t st)
+{
+    switch (up.nr) {
+    case -1: return launch_hydro_cfl_nr<-1>(ctx, U, A, up, cfl_scratch, st);
+    case 0: return launch_hydro_cfl_nr<0>(ctx, U, A, up, cfl_scratch, st);
+    case 1: return launch_hydro_cfl_nr<1>(ctx, U, A, up, cfl_scratch, st);
+    case 2: return launch_hydro_cfl_nr<2>(ctx, U, A, up, cfl_scratch, st);
+    case 3: return launch_hydro_cfl_nr<3>(ctx, U, A, up, cfl_scratch, st);
+    }
+    return CST_EINVAL;
 }
 
 template <int NR>

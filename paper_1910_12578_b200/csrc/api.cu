@@ -161,6 +161,28 @@ extern "C" int cst_advance_A_update(cst_ctx* c, const double* U_m, double* A_new
     return check_launch(launch_advance_A(c, U_m, A_new_m, U_next, dt_m, A_old_m, q, true, (cudaStream_t)stream));
 }
 
+extern "C" int cst_advance_A_update_cfl(cst_ctx* c, const double* U_m, double* A_new_m, double* U_next,
+                                        double dt_m, const double* A_old_m,
+                                        int nquad, const double* const* A_quad, const double* w_quad,
+                                        double cfl, double* dt_out_dev, void* stream)
+{
+    if (!c || !U_m || !A_new_m || !U_next || !A_old_m || !dt_out_dev || !(cfl > 0)) return CST_EINVAL;
+    if (U_next == U_m) return CST_EINVAL;
+    QuadArgs q;
+    int rc = make_quad(nquad, A_quad, w_quad, q);
+    if (rc) return rc;
+    const void* in[2 + CST_MAX_QUAD] = { U_m, A_old_m };
+    for (int n = 0; n < nquad; ++n) in[2 + n] = q.A[n];
+    for (int n = 0; n < 2 + nquad; ++n) {
+        if (in[n] == (const void*)U_next) return CST_EINVAL;
+        if (n != 0 && in[n] == (const void*)A_new_m) continue;
+        if (in[n] == (const void*)A_new_m) return CST_EINVAL;
+    }
+    if ((const void*)U_next == (const void*)A_new_m) return CST_EINVAL;
+    return check_launch(launch_advance_A_cfl(c, U_m, A_new_m, U_next, dt_m, A_old_m, q, true, cfl, dt_out_dev,
+                                             (cudaStream_t)stream));
+}
+
 extern "C" int cst_cfl_dt_device(cst_ctx* c, const double* U, double cfl, double* dt_out_dev, void* stream)
 {
     if (!c || !U || !dt_out_dev || !(cfl > 0)) return CST_EINVAL;

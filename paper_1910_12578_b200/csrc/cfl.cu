@@ -109,6 +109,20 @@ __global__ void k_cfl_final(const double* scratch, double cfl, double* dt_out)
     *dt_out = cfl / scratch[0];
 }
 
+// the two ends of the reduction on their own, for the advance call that folds the max into its z sweep (advect.cu)
+int launch_cfl_reset(cst_ctx* ctx, cudaStream_t st)
+{
+    k_cfl_reset<<<1, 1, 0, st>>>(ctx->d_scratch);
+    ctx->launches++;
+    return cudaGetLastError() == cudaSuccess ? CST_OK : CST_ECUDA;
+}
+int launch_cfl_final(cst_ctx* ctx, double cfl, double* dt_out_dev, cudaStream_t st)
+{
+    k_cfl_final<<<1, 1, 0, st>>>(ctx->d_scratch, cfl, dt_out_dev);
+    ctx->launches++;
+    return cudaGetLastError() == cudaSuccess ? CST_OK : CST_ECUDA;
+}
+
 int launch_cfl(cst_ctx* ctx, const double* U, double cfl, double* dt_out_dev, cudaStream_t st)
 {
     const Geom& g = ctx->g;

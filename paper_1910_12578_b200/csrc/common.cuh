@@ -66,7 +66,13 @@ __host__ __device__ inline long long aidx(const Geom& g, int b, int c, int k, in
 // launchers (one per source file)
 int launch_fill_ghosts(cst_ctx*, double* U, cudaStream_t);
 int launch_advance_A(cst_ctx*, const double* U, double* A, double* U_next, double dt_m,
-                     const double* A_old_m, const QuadArgs& q, bool fused, cudaStream_t);
+                     const double* A_old_m, const QuadArgs& q, bool fused, cudaStream_t, double* cfl_scratch = nullptr);
+int launch_advance_A_cfl(cst_ctx*, const double* U, double* A, double* U_next, double dt_m, const double* A_old_m,
+                         const QuadArgs& q, bool fused, double cfl, double* dt_out_dev, cudaStream_t);
+int launch_advect_hydro_cfl(cst_ctx*, const double* U, double* A, const UpdArgs& up, double* cfl_scratch, cudaStream_t);
+bool hydro_cfl_eligible(const cst_ctx*, const double* U);
+int launch_cfl_reset(cst_ctx*, cudaStream_t);
+int launch_cfl_final(cst_ctx*, double cfl, double* dt_out_dev, cudaStream_t);
 int launch_advect_hydro(cst_ctx*, const double* U, double* A, const UpdArgs& up, cudaStream_t);
 int launch_advect_species(cst_ctx*, const double* U, double* A, const UpdArgs& up, cudaStream_t);
 long long workspace_bytes(const cst_ctx* ctx);

@@ -94,3 +94,28 @@ def test_tuner_keeps_a_valid_variant_and_valid_outputs():
     orc.sdc_update(cfg, Uno, U, 1e-3, Ao, Ao, [Ao, Ao], [5e-4, 5e-4])
     assert comp_err(Un.cpu().numpy(), Uno).max() <= TOL
     ctx.destroy()
+
+
+@pytest.mark.parametrize("n,nb,ns", [
+    ((32, 16, 16), (1, 1, 1), 3),          # full tiles: the CFL max is gathered inside the hydro kernel's z sweep
+    ((16, 16, 32), (2, 1, 1), 0),          # boxes, no species
+    ((20, 12, 9), (1, 1, 1), 2),           # ragged tiles: the two calls run back to back
+])
+def test_fused_cfl_call_matches_the_separate_calls_and_the_oracle(n, nb, ns):
+    cfg = small_cfg(n=n, nb=nb, nspec=ns, gamma=5 / 3, bc=(0, 1, 2), grav=(0.0, 0.0, -0.2))
+    U = orc.fill_ghosts(cfg, wl.random_state(cfg, 113))
+    dt_o = orc.cfl_dt(cfg, U, 0.4)
+    ctx = Context(cfg)
+    Ud = dev(U)
+    dt = 1e-3
+    A0 = torch.full(wl.a_shape(cfg), float("nan"), dtype=torch.float64, device=DEV)
+    Un0 = torch.full(wl.u_shape(cfg), 3.0, dtype=torch.float64, device=DEV)
+    ctx.advance_A_update(Ud, A0, Un0, dt, A0, [A0, A0], [0.5 * dt, 0.5 * dt])
+    A1, Un1 = torch.full_like(A0, float("nan")), torch.full_like(Un0, 3.0)
+    dtd = torch.zeros(1, dtype=torch.float64, device=DEV)
+    for _ in range(2):                                       # twice: the reduction cell is reset by every call
+        ctx.advance_A_update_cfl(Ud, A1, Un1, dt, A1, [A1, A1], [0.5 * dt, 0.5 * dt], 0.4, dtd)
+    assert np.array_equal(A1.cpu().numpy(), A0.cpu().numpy()) and np.array_equal(Un1.cpu().numpy(), Un0.cpu().numpy())
+    assert abs(float(dtd.cpu()[0]) - dt_o) <= 1e-14 * dt_o
+    assert abs(ctx.cfl_dt(Ud, 0.4) - dt_o) <= 1e-14 * dt_o
+    ctx.destroy()
