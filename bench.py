@@ -48,6 +48,9 @@ def parse():
     ap.add_argument("--no-tune", action="store_true", help="keep species-kernel variant 0 instead of timing the variants")
     ap.add_argument("--exchange", default="sendrecv", choices=["sendrecv", "p2p"],
                     help="multi-GPU ghost exchange: NCCL send/recv of packed messages, or direct stores into peer-mapped memory")
+    ap.add_argument("--next", action="store_true",
+                    help="time the kernels of the rows beyond S0-S6 (reactions, diffusion, flattening, fourth order, CTU) "
+                         "on configs[3]'s distribution at 256^3 instead of the headline path; one JSON line, 1 GPU")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     return ap.parse_args()
@@ -490,6 +493,99 @@ def measure(cfg, args, rank, world, local, dev, want_e2e, want_cpu_baseline):
     return line
 
 
+def measure_next(args, dev):
+    """--next: each operator of SURVEY 8(f) on one mid-size box (configs[3]'s distribution, 256^3 by default, NVAR = 18),
+    device-resident, CUDA events, with the strict algorithmic byte count (what the operator must read and write once)
+    beside the time, and the oracle's twin timed on a 48^3 sample.  None of these kernels is tuned: the fractions say
+    how far the straightforward multi-pass versions are from a fused treatment."""
+    import torch
+    from paper_1910_12578_b200 import Context
+    from oracle import orc
+    n = args.n or 256
+    cfg = wl.make_config(3, n=n)
+    N, zones = wl.nvar(cfg), wl.nzones(cfg)
+    peak, peak_src = measured_peaks()
+    U_host = torch.zeros(wl.u_shape(cfg), dtype=torch.float64)
+    fill_host_state(cfg, U_host.numpy())
+    U = U_host.to(dev)
+    mk = lambda: torch.zeros(wl.a_shape(cfg), dtype=torch.float64, device=dev)
+    A, A2, R, R2 = mk(), mk(), mk(), mk()
+    Un = U.clone()
+    scfg = wl.make_config(3, n=48)
+    Us = orc.fill_ghosts(scfg, wl.initial_state(scfg))
+    react = wl.react_params(cfg["nspec"])
+    Zs = np.zeros(wl.a_shape(scfg))
+    ev = lambda: torch.cuda.Event(enable_timing=True)
+    out = {}
+
+    def timed(name, fn, alg_bytes_per_zone, oracle_fn, launches_ctx):
+        for _ in range(max(1, args.warmup)):
+            fn()
+        torch.cuda.synchronize()
+        l0 = launches_ctx.launch_count()
+        e0, e1 = ev(), ev()
+        e0.record()
+        for _ in range(args.steps):
+            fn()
+        e1.record()
+        torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1) / args.steps
+        t0 = time.perf_counter()
+        oracle_fn()
+        sec = time.perf_counter() - t0
+        gbs = alg_bytes_per_zone * zones / (ms * 1e-3) / 1e9
+        out[name] = {"ms": ms, "zone_updates_per_s": zones / (ms * 1e-3), "alg_bytes_per_zone": alg_bytes_per_zone,
+                     "achieved_gbs": gbs, "frac_of_hbm_peak": gbs / peak,
+                     "launches_per_call": (launches_ctx.launch_count() - l0) // args.steps,
+                     "oracle_zone_updates_per_s": wl.nzones(scfg) / sec}
+
+    ctx = Context(cfg)
+    ctx.fill_ghosts(U)
+    dt = ctx.cfl_dt(U, 0.5)
+    ctx.advance_A(U, A)
+    # NEXT-3: the implicit node update (reads U_m, A_new, A_old, R_old, 2 x (A_q + R_q); writes U_next, R_new)
+    ctx.set_reactions(react)
+    ctx.react_R(U, R)
+    timed("sdc_update_react", lambda: ctx.sdc_update_react(Un, U, dt, A, A, R, [A, A], [R, R], [0.5 * dt, 0.5 * dt], R2),
+          10 * N * 8, lambda: orc.sdc_update_react(scfg, react, Us.copy(), Us, 1e-3, Zs, Zs, orc.react_R(scfg, react, Us),
+                                                   [Zs, Zs], [Zs, Zs], [5e-4, 5e-4]), ctx)
+    # NEXT-4: the diffusion term alone = (A with it) - (A without it): time both, report the difference
+    timed("advance_A (reference point: second-order path)", lambda: ctx.advance_A(U, A2), 2 * N * 8,
+          lambda: orc.advance_A(scfg, Us), ctx)
+    ctx.set_diffusion(0.01, 1.5)
+    timed("advance_A + diffusion", lambda: ctx.advance_A(U, A2), 2 * N * 8 , lambda: orc.advance_A_diffuse(scfg, 0.01, 1.5, Us), ctx)
+    ctx.set_diffusion(0.0, 1.5)
+    ctx.destroy()
+    del ctx
+    # NEXT-2 (i): flattening (general kernels)
+    ctx = Context(cfg, workspace=None)
+    ctx.set_flattening(True)
+    ctx.set_workspace(torch.empty(ctx.workspace_bytes(), dtype=torch.uint8, device=dev))
+    timed("advance_A + flattening", lambda: ctx.advance_A(U, A2), 2 * N * 8, lambda: orc.advance_A_flat(scfg, Us), ctx)
+    ctx.destroy()
+    del ctx
+    torch.cuda.empty_cache()
+    # NEXT-1: fourth order
+    ctx = Context(cfg, workspace=None)
+    ctx.set_order(4)
+    ws = torch.empty(ctx.workspace_bytes(), dtype=torch.uint8, device=dev)
+    ctx.set_workspace(ws)
+    timed("advance_A order 4", lambda: ctx.advance_A(U, A2), 2 * N * 8, lambda: orc.advance_A4(scfg, Us), ctx)
+    ctx.destroy()
+    del ctx, ws
+    torch.cuda.empty_cache()
+    # NEXT-2 (ii): CTU
+    ctx = Context(cfg)
+    ws = torch.empty(ctx.ctu_workspace_bytes(), dtype=torch.uint8, device=dev)
+    timed("advance_ctu", lambda: ctx.advance_ctu(U, dt, A2, ws), 2 * N * 8, lambda: orc.advance_ctu(scfg, Us, 1e-3), ctx)
+    ctx.destroy()
+    return {"metric": "kernels of the rows beyond S0-S6 (SURVEY 8(f)): ms per call, zone-updates/s, strict algorithmic bytes",
+            "unit": "ms", "n_gpus": 1, "steps": args.steps, "warmup": max(1, args.warmup), "dtype": "f64", "data": "synthetic",
+            "config": {"workload": f"configs[3] distribution on one {n}^3 box, NVAR={N}", "zones": zones,
+                       "oracle_sample": "48^3 box, one call, all host threads"},
+            "peak_gbs": peak, "peak_source": peak_src, "kernels": out}
+
+
 def main():
     args = parse()
     rank = int(os.environ.get("RANK", "0"))
@@ -511,6 +607,13 @@ def main():
     dev = torch.device("cuda", local)
     if world > 1:
         dist.init_process_group("nccl", device_id=dev)
+
+    if getattr(args, "next", False):
+        if rank == 0:
+            print(json.dumps(measure_next(args, dev)), flush=True)
+        if world > 1:
+            dist.destroy_process_group()
+        return
 
     line = measure(cfg, args, rank, world, local, dev, not args.no_e2e, not args.no_cpu_baseline)
     if args.workload is None and not args.n:
