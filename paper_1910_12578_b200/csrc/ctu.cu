@@ -212,14 +212,14 @@ kctu_flux(Geom g, CtuArr arr, CtuRange rg, int T1, int T2, double c1, double c2,
         double wl[5], wr[5], F[5], rol, rnl, ror, rnr;
         ctu_corrected<MODE>(g, arr, 3 + D, z - stD, T1, T2, c1, c2, st1, st2, f1, f2, wl, rol, rnl);     // plus state of the low neighbour
         ctu_corrected<MODE>(g, arr, D, z, T1, T2, c1, c2, st1, st2, f1, f2, wr, ror, rnr);               // minus state of this zone
-        hllc<D>(g, wl, wr, F);
+        const bool left = hllc_ieee<D>(g, wl, wr, F);
         double* __restrict__ Fo = arr.a[fout] + z;
 #pragma unroll
         for (int v = 0; v < 5; ++v) Fo[v * g.comp_g] = F[v];
         for (int s = 5; s < g.nvar; ++s) {
-            const double X = sign_bit(F[0])
-                ? ctu_corrected_x<MODE>(g, arr, D, z, s, c1, c2, st1, st2, f1, f2, ror, rnr)
-                : ctu_corrected_x<MODE>(g, arr, 3 + D, z - stD, s, c1, c2, st1, st2, f1, f2, rol, rnl);
+            const double X = left
+                ? ctu_corrected_x<MODE>(g, arr, 3 + D, z - stD, s, c1, c2, st1, st2, f1, f2, rol, rnl)
+                : ctu_corrected_x<MODE>(g, arr, D, z, s, c1, c2, st1, st2, f1, f2, ror, rnr);
             Fo[s * g.comp_g] = F[0] * X;
         }
     }

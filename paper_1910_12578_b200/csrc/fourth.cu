@@ -240,11 +240,11 @@ k4_fa(Geom g, Face4 fa, const double* __restrict__ WL, const double* __restrict_
 #pragma unroll
         for (int c = 0; c < 5; ++c) { wl[c] = WL[w + c * fa.per_comp]; wr[c] = WR[w + c * fa.per_comp]; }
         floor4(g, wl); floor4(g, wr);
-        hllc<D>(g, wl, wr, F);
+        const bool left = hllc_ieee<D>(g, wl, wr, F);
 #pragma unroll
         for (int c = 0; c < 5; ++c) Fa[w + c * fa.per_comp] = F[c];
-        for (int s = 5; s < g.nvar; ++s)               // Q8: mass flux x upwind X (the sign of F[rho] picks the side)
-            Fa[w + s * fa.per_comp] = F[0] * (sign_bit(F[0]) ? WR[w + s * fa.per_comp] : WL[w + s * fa.per_comp]);
+        for (int s = 5; s < g.nvar; ++s)               // Q8: mass flux x upwind X
+            Fa[w + s * fa.per_comp] = F[0] * (left ? WL[w + s * fa.per_comp] : WR[w + s * fa.per_comp]);
     }
 }
 
@@ -285,7 +285,7 @@ k4_favg(Geom g, Face4 fa, const double* __restrict__ WL, const double* __restric
             wr[c] = sub_rn(rgt[0], __dmul_rn(R24, lap_t(rgt, sa, sb)));
         }
         floor4(g, wl); floor4(g, wr);
-        hllc<D>(g, wl, wr, Fc);
+        const bool left = hllc_ieee<D>(g, wl, wr, Fc);
 #pragma unroll
         for (int c = 0; c < 5; ++c)
             Fv[w + c * fa.per_comp] = Fc[c] + R24 * lap_t(Fa + w + c * fa.per_comp, sa, sb);           // G7
@@ -294,7 +294,7 @@ k4_favg(Geom g, Face4 fa, const double* __restrict__ WL, const double* __restric
             const double* rgt = WR + w + s * fa.per_comp;
             const double xl = sub_rn(l[0], __dmul_rn(R24, lap_t(l, sa, sb)));
             const double xr = sub_rn(rgt[0], __dmul_rn(R24, lap_t(rgt, sa, sb)));
-            const double fc = Fc[0] * (sign_bit(Fc[0]) ? xr : xl);
+            const double fc = Fc[0] * (left ? xl : xr);
             Fv[w + s * fa.per_comp] = fc + R24 * lap_t(Fa + w + s * fa.per_comp, sa, sb);
         }
     }
