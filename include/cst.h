@@ -8,6 +8,10 @@
  *          fluxes along with hydrodynamic sources"; evaluated at a node time)
  *   S5  the SDC node update, Eq. (2), R = 0
  *   S6  the CFL time step                       (BASELINE.json north_star; Q20)
+ * Beyond that path (each documented at its declaration below): the box lattice sharded over ranks
+ * (cst_set_sublattice, cst_exchange_*), reactions R != 0 (cst_sdc_update_react), explicit diffusion (cst_set_diffusion),
+ * shock flattening (cst_set_flattening), the fourth-order operator (cst_set_order), the unsplit CTU PPM operator
+ * (cst_advance_ctu), kernel variants chosen by measurement (cst_tune_advance), S1-S6 in one call (cst_advance_A_update_cfl).
  * Every step runs in hand-written CUDA kernels for sm_100a; there is no CPU fallback.
  *
  * LAYOUT.  All arrays are fp64, C-contiguous, in DEVICE memory:

@@ -523,4 +523,4 @@ extern "C" const char* cst_strerror(int code)
     }
 }
 
-extern "C" const char* cst_version(void) { return "libcst 0.2 (sm_100a)"; }
+extern "C" const char* cst_version(void) { return "libcst 0.3 (sm_100a)"; }
