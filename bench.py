@@ -291,7 +291,7 @@ def measure(cfg, args, rank, world, local, dev, want_e2e, want_cpu_baseline):
             v, ms_v = ctx.tune_advance(U, A_new, U_next, dt, A_old0, [A_old0, A_old1], w, repeats=2)
             tuned = {"species_variant": v, "species_split": ctx.get_species_split() or 3, "ms": ms_v,
                      "note": "cst_tune_advance: ms of the fused advance (hydro + species kernels), min of 2 runs: variants "
-                             "0, 1, 2 with three CTAs per tile, then the winner with 2 and 4"}
+                             "0, 1, 2, 3 with three CTAs per tile, then the winner with 2 and 4"}
         except Exception as exc:
             ctx.set_variant(0)
             tuned = {"species_variant": 0, "ms": None, "note": f"tuning failed ({exc}); variant 0"}

@@ -152,15 +152,17 @@ int cst_sdc_update(cst_ctx* ctx, double* U_next, const double* U_m, double dt_m,
  * performs the same operations in the same order, so results are bit-identical.
  *   0  (default) conversion phase + three sweeps + write-out phase per species: the kernel that has been profiled;
  *   1  X = rho X / rho formed inside the x sweep (no conversion phase);
- *   2  as 1, and each component is written out from its own z sweep (no write-out phase).
- * cst_set_variant selects one (CST_EINVAL outside 0..2); cst_get_variant returns the current one.
+ *   2  as 1, and each component is written out from its own z sweep (no write-out phase);
+ *   3  as 2, with the L2 prefetches (next species' tile, operands of the update) issued one sweep instead of one to
+ *      two sweeps ahead of their use (less of the prefetched data is evicted again before it is read).
+ * cst_set_variant selects one (CST_EINVAL outside 0..3); cst_get_variant returns the current one.
  * cst_set_species_split: how many consecutive CTAs share one tile, each taking a contiguous share of the species
  * (0 = the default, 3; at most 8; never more than nspec).  Does not change results either.
  * cst_tune_advance runs cst_advance_A_update (same arguments, same rules) `repeats` + 1 times with every variant on
  * the caller's buffers, times each with CUDA events on `stream` (minimum over the repeats; the first run of a
  * configuration is a warm-up), then tries 2 and 4 CTAs per tile with the winner, keeps the fastest configuration for all
- * later calls and leaves A_new_m / U_next valid; ms_out (HOST, 5 floats, may be NULL) receives the times in
- * milliseconds: variants 0, 1, 2 at the default split, then the winner at split 2 and 4.  Synchronises the stream.
+ * later calls and leaves A_new_m / U_next valid; ms_out (HOST, 6 floats, may be NULL) receives the times in
+ * milliseconds: variants 0, 1, 2, 3 at the default split, then the winner at split 2 and 4.  Synchronises the stream.
  * Measurement, not arithmetic: which configuration wins depends on the device and the box shape. */
 int cst_set_variant(cst_ctx* ctx, int species_variant);
 int cst_get_variant(const cst_ctx* ctx);

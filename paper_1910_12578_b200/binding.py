@@ -300,9 +300,9 @@ class Context:
 
     def tune_advance(self, U_m, A_new_m, U_next, dt_m, A_old_m, A_quad, w_quad, repeats=2, stream=None):
         """cst_tune_advance: times the fused advance with every species-kernel variant, keeps the fastest.
-        -> (chosen variant, [ms of variant 0, 1, 2 at the default split, ms of the winner at split 2 and 4])."""
+        -> (chosen variant, [ms of variant 0, 1, 2, 3 at the default split, ms of the winner at split 2 and 4])."""
         n, arr, w = self._quad(A_quad, w_quad)
-        ms = (C.c_float * 5)()
+        ms = (C.c_float * 6)()
         self._check(self.lib.cst_tune_advance(self._h, _ptr(U_m), _ptr(A_new_m), _ptr(U_next), float(dt_m), _ptr(A_old_m),
                                               n, arr, w, int(repeats), ms, _stream(stream)), "cst_tune_advance")
         return self.get_variant(), [float(x) for x in ms]

@@ -205,6 +205,10 @@ static int launch_species_nr(cst_ctx* ctx, const double* U, double* A, const Upd
             if (cudaFuncSetAttribute(k_advect_species_tma_v<NR, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, SPT_SMEM) != cudaSuccess)
                 return CST_ECUDA;
             k_advect_species_tma_v<NR, 2><<<grid, NTHR, SPT_SMEM, st>>>(g, tg, maps, U, A, rinv, Fm, up, split);
+        } else if (ctx->species_variant == 3) {
+            if (cudaFuncSetAttribute(k_advect_species_tma_v<NR, 3>, cudaFuncAttributeMaxDynamicSharedMemorySize, SPT_SMEM) != cudaSuccess)
+                return CST_ECUDA;
+            k_advect_species_tma_v<NR, 3><<<grid, NTHR, SPT_SMEM, st>>>(g, tg, maps, U, A, rinv, Fm, up, split);
         } else {
             k_advect_species_tma<NR><<<grid, NTHR, SPT_SMEM, st>>>(g, tg, maps, U, A, rinv, Fm, up, split);
         }

@@ -239,7 +239,7 @@ extern "C" int cst_step_host(cst_ctx* c, const double* U_host, double* A_host, d
 
 extern "C" int cst_set_variant(cst_ctx* c, int species_variant)
 {
-    if (!c || species_variant < 0 || species_variant > 2) return CST_EINVAL;
+    if (!c || species_variant < 0 || species_variant > 3) return CST_EINVAL;
     c->species_variant = species_variant;
     return CST_OK;
 }
@@ -270,7 +270,7 @@ extern "C" int cst_tune_advance(cst_ctx* c, const double* U_m, double* A_new_m, 
     c->timing = 0;
     int best = 0, rc = CST_OK;
     float best_ms = 0.f;
-    for (int v = 0; v <= 2 && rc == CST_OK; ++v) {
+    for (int v = 0; v <= 3 && rc == CST_OK; ++v) {
         c->species_variant = v;
         float ms_v = 0.f;
         for (int n = 0; n <= repeats && rc == CST_OK; ++n) {          // the first run of a variant is a warm-up
@@ -302,7 +302,7 @@ extern "C" int cst_tune_advance(cst_ctx* c, const double* U_m, double* A_new_m, 
             cudaEventElapsedTime(&ms, e0, e1);
             if (n == 1 || (n > 1 && ms < ms_s)) ms_s = ms;
         }
-        if (ms_out) ms_out[3 + (sp == 4)] = ms_s;
+        if (ms_out) ms_out[4 + (sp == 4)] = ms_s;
         if (rc == CST_OK && ms_s < best_ms) { best_split = sp; best_ms = ms_s; }
     }
     c->species_split = (rc == CST_OK) ? best_split : 0;

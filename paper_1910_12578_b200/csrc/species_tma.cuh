@@ -547,7 +547,7 @@ __device__ __forceinline__ void spt_tile_v(const Geom& g, const TileCoord& tc, c
                                            const double* __restrict__ fm_tile, double* __restrict__ A, const UpdArgs& up,
                                            double* __restrict__ sm, const int s_begin, const int s_end)
 {
-    constexpr bool ZOUT = (V == 2);
+    constexpr bool ZOUT = (V >= 2), LATE = (V == 3);     // V = 3: as 2, with the L2 prefetches issued one sweep ahead of their use
     const int ng = CST_NG;
     double* Xs = sm;                                  // [SPT_XTILE]
     double* PB = sm + SPT_XTILE;                      // [SPT_TILE]
@@ -581,7 +581,7 @@ __device__ __forceinline__ void spt_tile_v(const Geom& g, const TileCoord& tc, c
         const unsigned long long keep = last ? spt_policy_stream() : spt_policy_keep();
         const double* Us = Ub + (long long)c * g.comp_g;
         if (!ZOUT && n > 0) spt_write_out<NR>(g, tc, PB, A, up, c - 1);
-        if (tid == 0) {
+        if (tid == 0 && !LATE) {
             if (!last) tma_prefetch_3d(&maps.u, tx, ty, zc0 + (c + 1) * g.ez);
             if (NR > 0) {
 #pragma unroll
@@ -596,12 +596,17 @@ __device__ __forceinline__ void spt_tile_v(const Geom& g, const TileCoord& tc, c
         // ---- x sweep (+ conversion)
         spt_sweep_x_conv(Xs + spt_xbase<0>(a, b), PB + spt_pbase<0>(a, b), fm, rrow, nrdx, keep);
         __syncthreads();
+        if (LATE && tid == 0 && NR > 0) {             // operands of this component's update: read by the z sweep
+#pragma unroll
+            for (int r = 0; r < NR; ++r) tma_prefetch_3d(&maps.p[r], tc.i0, tc.j0, za0 + c * g.nz);
+        }
         // ---- y sweep
 #pragma unroll
         for (int m = 0; m < 6; ++m) hx[m] = hr.u[m] * hr.r[m];
         spt_halo_load(g, tc, 2, Us, rinv_b, hr, keep);
         spt_sweep_yz<1>(Xs + spt_xbase<1>(a, b), PB + spt_pbase<1>(a, b), fm + (TILE + 1) * NTHR, hx, nrdy, keep);
         __syncthreads();
+        if (LATE && tid == 0 && !last) tma_prefetch_3d(&maps.u, tx, ty, zc0 + (c + 1) * g.ez);   // the tile loaded after the z sweep
         // ---- z sweep (+ write-out)
 #pragma unroll
         for (int m = 0; m < 6; ++m) hx[m] = hr.u[m] * hr.r[m];

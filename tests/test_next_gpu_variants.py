@@ -39,11 +39,11 @@ def test_variants_match_oracle_and_each_other(n, nb, ns, bc):
     Ud, Pd = dev(U), [dev(p) for p in P]
     ctx = Context(cfg)
     with pytest.raises(CstError):
-        ctx.set_variant(3)
+        ctx.set_variant(4)
     # update arities: plain A (NR = -1), forward Euler (0 external arrays), 1, 2, 3 external arrays
     cases = {"plain": None, "nr0": ("self", []), "nr1": (0, [0]), "nr2": (0, [0, 1]), "nr3": (0, [1, 2])}
     ref = {}
-    for v in (0, 1, 2):
+    for v in (0, 1, 2, 3):
         ctx.set_variant(v)
         assert ctx.get_variant() == v
         for name, case in cases.items():
@@ -85,10 +85,10 @@ def test_tuner_keeps_a_valid_variant_and_valid_outputs():
     A = torch.full(wl.a_shape(cfg), float("nan"), dtype=torch.float64, device=DEV)
     Un = torch.full(wl.u_shape(cfg), 3.0, dtype=torch.float64, device=DEV)
     v, ms = ctx.tune_advance(Ud, A, Un, 1e-3, A, [A, A], [5e-4, 5e-4], repeats=1)
-    assert v in (0, 1, 2) and len(ms) == 5 and all(m > 0 for m in ms) and ms[v] == min(ms[:3])
+    assert v in (0, 1, 2, 3) and len(ms) == 6 and all(m > 0 for m in ms) and ms[v] == min(ms[:4])
     assert ctx.get_species_split() in (0, 2, 4)
     if ctx.get_species_split():
-        assert ms[3 + (ctx.get_species_split() == 4)] == min(ms)
+        assert ms[4 + (ctx.get_species_split() == 4)] == min(ms)
     assert comp_err(A.cpu().numpy(), Ao).max() <= TOL
     Uno = np.full_like(U, 3.0)
     orc.sdc_update(cfg, Uno, U, 1e-3, Ao, Ao, [Ao, Ao], [5e-4, 5e-4])
