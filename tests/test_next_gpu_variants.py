@@ -119,3 +119,66 @@ def test_fused_cfl_call_matches_the_separate_calls_and_the_oracle(n, nb, ns):
     assert abs(float(dtd.cpu()[0]) - dt_o) <= 1e-14 * dt_o
     assert abs(ctx.cfl_dt(Ud, 0.4) - dt_o) <= 1e-14 * dt_o
     ctx.destroy()
+
+
+# ------------------------------------------------------------ the launch configurations bench.py may time, at full size ----
+def checksums(t):
+    """two order-independent integer checksums of the BIT PATTERNS of a float64 tensor (wrap-around sums)"""
+    a = b = 0
+    for box in t:                              # component by component: the shifted copy stays small
+        for comp in box:
+            v = comp.reshape(-1).view(torch.int64)
+            a += int(v.sum())
+            b += int((v >> 11).sum())
+    return a % (1 << 64), b % (1 << 64)
+
+
+def variants_agree_bitwise(cfg):
+    """Every species-kernel variant, every number of CTAs per tile the tuner tries, and the fused-CFL call produce the
+    same bits as variant 0 with separate calls -- whose every zone tests/test_gpu_fullsize.py compares with the oracle."""
+    from test_gpu_fullsize import device_state
+    ctx = Context(cfg)
+    U = device_state(cfg)
+    ctx.fill_ghosts(U)
+    dt = ctx.cfl_dt(U, 0.5)
+    ash = wl.a_shape(cfg)
+    A0 = torch.empty(ash, dtype=torch.float64, device=DEV)
+    ctx.advance_A(U, A0)
+    A1 = A0 * 0.9
+    A = torch.empty(ash, dtype=torch.float64, device=DEV)
+    Un = torch.empty(wl.u_shape(cfg), dtype=torch.float64, device=DEV)
+    w = [0.5 * dt, 0.5 * dt]
+    ref = None
+    for variant, split, fused in [(0, 0, False), (1, 0, False), (2, 0, False), (3, 0, False), (2, 2, False), (2, 4, False),
+                                  (0, 0, True), (2, 0, True)]:
+        ctx.set_variant(variant)
+        ctx.set_species_split(split)
+        A.fill_(float("nan"))
+        Un.fill_(3.0)
+        if fused:
+            dtd = torch.zeros(1, dtype=torch.float64, device=DEV)
+            ctx.advance_A_update_cfl(U, A, Un, dt, A0, [A0, A1], w, 0.5, dtd)
+            assert float(dtd.cpu()[0]) == dt or abs(float(dtd.cpu()[0]) - dt) <= 1e-14 * dt
+        else:
+            ctx.advance_A_update(U, A, Un, dt, A0, [A0, A1], w)
+        torch.cuda.synchronize()
+        got = (checksums(A), checksums(Un))
+        if ref is None:
+            assert torch.isfinite(A).all()
+            ref = got
+        assert got == ref, (variant, split, fused)
+    ctx.destroy()
+
+
+def test_variants_agree_bitwise_at_full_size_configs3():
+    import gc
+    gc.collect()
+    torch.cuda.empty_cache()
+    free, _ = torch.cuda.mem_get_info()
+    if free < 112e9:
+        pytest.skip(f"needs 112 GB of free device memory, has {free / 1e9:.0f}")
+    variants_agree_bitwise(wl.make_config(3))
+
+
+def test_variants_agree_bitwise_on_a_batch_of_boxes():
+    variants_agree_bitwise(wl.make_config(4, nb=(4, 2, 1)))          # 8 of configs[4]'s boxes (64^3, reflecting z, gravity)
