@@ -119,6 +119,32 @@ def test_plan_reproduces_the_global_ghost_fill(n, gnb, bc, part):
         assert np.array_equal(got[m5], expect[m5]), "exchanged ghost zones differ from the single-lattice fill"
 
 
+@pytest.mark.parametrize("n,gnb,bc,part", CASES[:5])
+def test_push_form_of_the_plan_reproduces_the_global_ghost_fill(n, gnb, bc, part):
+    """The send segments also name the destination (rbox, rlo): executing them as direct stores into the peers' arrays
+    (what cst_exchange_push does on the device) must give the same shells as pack + message + unpack."""
+    cfg = small_cfg(n=n, nb=gnb, nspec=1, bc=bc)
+    Ug = orc.fill_ghosts(cfg, wl.random_state(cfg, 33))
+    world = part[0] * part[1] * part[2]
+    loc = []
+    for r in range(world):
+        U = Ug[shard.local_boxes(cfg, part, r)].copy()
+        U[np.broadcast_to(remote_mask(cfg, part, r)[:, None], U.shape)] = np.nan
+        loc.append(U)
+    for s in range(world):
+        for seg in binding.exchange_plan(cfg, part, s, recv=False):
+            ext = tuple(seg.ext)
+            idx = [seg.lo[d] + seg.step[d] * np.arange(ext[d]) for d in range(3)]
+            blk = loc[s][seg.box][:, idx[2][:, None, None], idx[1][None, :, None], idx[0][None, None, :]].copy()
+            for d in range(3):
+                if seg.flip[d]:
+                    blk[1 + d] *= -1.0
+            sl = tuple(slice(seg.rlo[d], seg.rlo[d] + ext[d]) for d in (2, 1, 0))
+            loc[seg.peer][seg.rbox][(slice(None),) + sl] = blk
+    for r in range(world):
+        assert np.array_equal(loc[r], Ug[shard.local_boxes(cfg, part, r)]), r
+
+
 def test_message_sizes_agree_between_the_two_sides():
     cfg = small_cfg(n=(4, 6, 5), nb=(4, 2, 2), nspec=1, bc=(0, 2, 1))
     part = (2, 2, 1)
