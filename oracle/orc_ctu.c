@@ -37,6 +37,9 @@
  * 1-D Sod against the exact Riemann solution at CFL 0.8 (the acoustic part of C3); second-order convergence in 3-D at
  * CFL 0.8 where the method-of-lines operator with one Euler stage is unstable; conservation, A(uniform) = 0,
  * permutation / mirror invariance, box-lattice equivalence.
+ * Unpinned by the paper itself (it only names refs [15, 16]): the choice of reference state and of zone-centre
+ * eigenvectors in C3, the passive treatment of transverse velocities, the source placement of C4 / C8 -- conventions,
+ * fixed by the readings and pinned only through the properties above.
  * Shares no code with paper_1910_12578_b200/csrc.
  */
 #include <math.h>

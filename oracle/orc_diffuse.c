@@ -13,6 +13,7 @@
  * Pins (tests/test_oracle_diffuse.py): D of a uniform-temperature state is exactly zero; sum of D over a periodic
  * domain vanishes to roundoff; for T = T0 + a sin(2 pi m x / L) the result converges to -k_th (2 pi m / L)^2 (T - T0)
  * at second order; the discrete eigenvalue -k_th (2 - 2 cos(theta)) / dx^2 is met to roundoff.
+ * Unpinned by the paper itself: constant k_th and c_v (D1-D2 stand in for its conductivity tables).
  */
 #include <math.h>
 

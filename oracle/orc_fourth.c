@@ -41,6 +41,8 @@
  * an analytic smooth state (ratio -> 16 where the second-order path gives 4); A(uniform) = 0; conservation;
  * permutation / mirror invariance; box-lattice equivalence; limiter: smooth monotone data untouched, a step stays
  * monotone, smooth extremum keeps its height; the space-time scheme (3-node SDC, 4 iterations) at fourth order.
+ * Unpinned by the paper itself (it only names ref [12]): G4b-G5 as recalled here, the omission of the third-difference
+ * test, the flux form of G7 -- pinned only through the properties above.
  * Shares no code with paper_1910_12578_b200/csrc.
  */
 #include <math.h>

@@ -23,6 +23,7 @@
  * bookkeeping to roundoff, residual of the converged nonlinear solve, analytic Jacobian against finite differences,
  * and the order of the whole SDC iteration with R != 0 (2 for trapezoid, 4 for Simpson) against a tight-tolerance
  * ODE reference on a uniform state (where <A(U)> = 0 bitwise).
+ * Unpinned by the paper itself: the network (R1-R2 are synthetic stand-ins), the Newton controls of R3.
  * Shares no code with paper_1910_12578_b200/csrc.  Build: -O2 -ffp-contract=off (oracle/build.py).
  */
 #include <math.h>
