@@ -46,6 +46,8 @@ def parse():
                     help="time this config only (default: configs[3], then configs[4] under \"also\")")
     ap.add_argument("--n", type=int, default=None, help="override zones per box side (debug only; marks the line)")
     ap.add_argument("--no-tune", action="store_true", help="keep species-kernel variant 0 instead of timing the variants")
+    ap.add_argument("--probe", action="store_true",
+                    help="(internal) child process: check every tunable configuration bitwise against variant 0, print one JSON line")
     ap.add_argument("--exchange", default="sendrecv", choices=["sendrecv", "p2p"],
                     help="multi-GPU ghost exchange: NCCL send/recv of packed messages, or direct stores into peer-mapped memory")
     ap.add_argument("--next", action="store_true",
@@ -231,6 +233,91 @@ def sharded_config(cfg, world):
 
 
 # -------------------------------------------------------------------------------------- main ----
+def probe_child():
+    """Runs in a CHILD process before anything is timed (see probe_configurations): on two reduced versions of the timed
+    workloads -- configs[3] as one 128 x 128 x 64 box, configs[4] as 2 x 2 x 2 boxes of 64^3 -- every configuration the tuner
+    may pick (species variants 1-3, 2 / 3 / 4 CTAs per tile, the CFL reduction folded into the advance) must reproduce
+    variant 0 with the separate CFL pass BIT FOR BIT.  Prints {"variants_ok": b, "fused_cfl_ok": b, ...}.  The product
+    path only: no oracle here (the oracle comparison of the same configurations is tests/test_next_gpu_variants.py)."""
+    import torch
+    from paper_1910_12578_b200 import Context
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    out = {"variants_ok": True, "fused_cfl_ok": True, "checked": 0, "failed": []}
+    for index, kw in ((3, {"n": (128, 128, 64)}), (4, {"nb": (2, 2, 2)})):
+        cfg = wl.make_config(index, **kw)
+        U_host = np.zeros(wl.u_shape(cfg))
+        fill_host_state(cfg, U_host)
+        U = torch.from_numpy(U_host).to(dev)
+        ctx = Context(cfg)
+        ctx.fill_ghosts(U)
+        dt_dev = torch.zeros(1, dtype=torch.float64, device=dev)
+        ctx.cfl_dt_device(U, 0.5, dt_dev)
+        dt_ref = float(dt_dev.cpu()[0])
+        A0 = torch.zeros(wl.a_shape(cfg), dtype=torch.float64, device=dev)
+        ctx.advance_A(U, A0)
+        A1 = A0 * 0.9
+        w = [0.5 * dt_ref, 0.5 * dt_ref]
+
+        def run(variant, split, fused):
+            ctx.set_variant(variant)
+            ctx.set_species_split(split)
+            A = torch.full_like(A0, 7.0)
+            Un = U.clone()
+            dt_f = None
+            if fused:
+                dt_dev.zero_()
+                ctx.advance_A_update_cfl(U, A, Un, dt_ref, A0, [A0, A1], w, 0.5, dt_dev)
+                dt_f = float(dt_dev.cpu()[0])
+            else:
+                ctx.advance_A_update(U, A, Un, dt_ref, A0, [A0, A1], w)
+            torch.cuda.synchronize()
+            return A, Un, dt_f
+
+        A_ref, Un_ref, _ = run(0, 3, False)
+        if not bool(torch.isfinite(A_ref).all()):
+            raise SystemExit("probe: variant 0 gave a non-finite A")
+        for variant in (0, 1, 2, 3):
+            for split in (2, 3, 4):
+                for fused in (False, True):
+                    if (variant, split, fused) == (0, 3, False):
+                        continue
+                    A, Un, dt_f = run(variant, split, fused)
+                    same = torch.equal(A, A_ref) and torch.equal(Un, Un_ref)
+                    if fused:
+                        same = same and dt_f is not None and abs(dt_f - dt_ref) <= 1e-14 * dt_ref
+                    out["checked"] += 1
+                    if not same:
+                        out["failed"].append([cfg["name"], variant, split, fused])
+                        if fused:
+                            out["fused_cfl_ok"] = False
+                        else:
+                            out["variants_ok"] = False
+        ctx.destroy()
+    print("PROBE " + json.dumps(out), flush=True)
+
+
+def probe_configurations(local):
+    """None of the tunable configurations (cst_tune_advance's variants, the fused CFL step) is ever timed unless a child
+    process has first run all of them on THIS device and found them bit-identical to the default path: a kernel fault
+    in a variant then ends the child, not the benchmark, and the timed run keeps variant 0 with the separate CFL pass."""
+    bad = {"variants_ok": False, "fused_cfl_ok": False}
+    env = {k: v for k, v in os.environ.items() if k not in ("RANK", "WORLD_SIZE", "LOCAL_WORLD_SIZE", "MASTER_ADDR", "MASTER_PORT")}
+    env["LOCAL_RANK"] = str(local)
+    try:
+        r = subprocess.run([sys.executable, os.path.abspath(__file__), "--probe"], env=env, capture_output=True, text=True, timeout=900)
+    except Exception as exc:
+        return dict(bad, note=f"probe did not finish ({type(exc).__name__}); default path only")
+    for ln in r.stdout.splitlines():
+        if ln.startswith("PROBE "):
+            res = json.loads(ln[6:])
+            res["note"] = "every tunable configuration checked bitwise against variant 0 in a child process on this device"
+            return res
+    tail = (r.stderr or "").strip().splitlines()[-1:] or [""]
+    return dict(bad, note=f"probe exited {r.returncode} ({tail[0][:200]}); default path only")
+
+
 def measure(cfg, args, rank, world, local, dev, want_e2e, want_cpu_baseline):
     """Times one workload (W warm-up + K timed steps) and returns the JSON line as a dict (rank 0; None elsewhere).
     Every device buffer is local to this function, so the memory is free again when it returns."""
@@ -286,7 +373,10 @@ def measure(cfg, args, rank, world, local, dev, want_e2e, want_cpu_baseline):
     # kernel variants of the species half (cst_tune_advance): every variant is timed on these buffers before the
     # warm-up steps and the fastest is kept; all variants give bit-identical results (tests/test_next_gpu_variants.py)
     tuned = {"species_variant": 0, "ms": None, "note": "not tuned"}
-    if not getattr(args, "no_tune", False) and N > 5:
+    safe = getattr(args, "safe", {"variants_ok": False, "fused_cfl_ok": False})
+    if not safe["variants_ok"]:
+        tuned["note"] = "not tuned: " + str(safe.get("note", "no probe"))
+    if not getattr(args, "no_tune", False) and N > 5 and safe["variants_ok"]:
         try:
             v, ms_v = ctx.tune_advance(U, A_new, U_next, dt, A_old0, [A_old0, A_old1], w, repeats=2)
             tuned = {"species_variant": v, "species_split": ctx.get_species_split() or 3, "ms": ms_v,
@@ -327,7 +417,7 @@ def measure(cfg, args, rank, world, local, dev, want_e2e, want_cpu_baseline):
             dist.barrier()
         torch.cuda.synchronize()
 
-    if not getattr(args, "no_tune", False):
+    if not getattr(args, "no_tune", False) and safe["fused_cfl_ok"]:
         # the step with the CFL reduction folded into the advance against the step with the separate CFL pass: 3 runs each
         # after one untimed run, the faster composition is kept (same results: tests/test_next_gpu_variants.py)
         try:
@@ -486,7 +576,7 @@ def measure(cfg, args, rank, world, local, dev, want_e2e, want_cpu_baseline):
                            "parallelism": f"box lattice sharded over {world} ranks, bricks {part[0]}x{part[1]}x{part[2]}" if world > 1
                                           else "single GPU",
                            "ms_per_step_best": float(min(per_step)), "ms_per_step_median": float(np.median(per_step)),
-                           "tuned": tuned, "fused_cfl": fused_cfl, "debug_size_override": bool(args.n)},
+                           "tuned": tuned, "fused_cfl": fused_cfl, "probe": safe, "debug_size_override": bool(args.n)},
                 "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline,
                 "cpu_baseline": cpu_baseline}
     ctx.destroy()
@@ -594,6 +684,9 @@ def main():
     head = 3 if args.workload is None else args.workload
     cfg = wl.make_config(head, n=args.n) if args.n else wl.make_config(head)
 
+    if args.probe:
+        probe_child()
+        return
     if args.impl == "reference":
         run_reference(args, cfg, rank)
         return
@@ -605,8 +698,13 @@ def main():
         raise SystemExit("bench.py needs a CUDA device (no CPU fallback)")
     torch.cuda.set_device(local)
     dev = torch.device("cuda", local)
+    args.safe = {"variants_ok": False, "fused_cfl_ok": False, "note": "not probed"}
+    if not args.no_tune and not getattr(args, "next", False):
+        args.safe = probe_configurations(local)       # a child process per rank, before this one allocates anything
     if world > 1:
         dist.init_process_group("nccl", device_id=dev)
+        for key in ("variants_ok", "fused_cfl_ok"):   # a configuration is used only if every rank's device passed it
+            args.safe[key] = bool(allreduce_scalar(1.0 if args.safe[key] else 0.0, "min", dev, world) > 0.5)
 
     if getattr(args, "next", False):
         if rank == 0:
