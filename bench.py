@@ -306,7 +306,7 @@ def probe_configurations(local):
     env = {k: v for k, v in os.environ.items() if k not in ("RANK", "WORLD_SIZE", "LOCAL_WORLD_SIZE", "MASTER_ADDR", "MASTER_PORT")}
     env["LOCAL_RANK"] = str(local)
     try:
-        r = subprocess.run([sys.executable, os.path.abspath(__file__), "--probe"], env=env, capture_output=True, text=True, timeout=900)
+        r = subprocess.run([sys.executable, os.path.abspath(__file__), "--probe"], env=env, capture_output=True, text=True, timeout=420)
     except Exception as exc:
         return dict(bad, note=f"probe did not finish ({type(exc).__name__}); default path only")
     for ln in r.stdout.splitlines():
