@@ -110,6 +110,44 @@ def test_hllc_uses_pvrs_estimate_and_wave_speeds():
         assert np.allclose(F, Fe, rtol=1e-11, atol=1e-11 * np.abs(Fe).max())
 
 
+def test_hllc_on_mirror_image_states_a_reflecting_wall():
+    """The face of a reflecting wall sees W_R = mirror(W_L): the numerator of S* cancels exactly, S* = 0.  Subsonic
+    approach: S_L < 0 < S_R, the star flux with NO mass through the wall and the wall pressure p + rho u c q (Rankine-
+    Hugoniot across S_L).  Approach faster than the PVRS shock speed: S_L > 0 > S_R, and the textbook's first test
+    (0 <= S_L: F = F_L, Toro (10.71)) decides -- the side S* >= 0 picks at S* = 0.  The CUDA path must take the same
+    side whatever the compiler fuses (tests/test_gpu_edge.py test_supersonic_flow_into_reflecting_walls)."""
+    g = 5.0 / 3.0
+    rng = np.random.default_rng(31)
+    seen = [0, 0]
+    for _ in range(200):
+        rho, p = np.exp(rng.normal()), np.exp(rng.normal())
+        c = np.sqrt(g * p / rho)
+        u = c * rng.uniform(0.05, 4.0)
+        v, w = rng.normal(), rng.normal()
+        for d in range(3):
+            WL = np.array([rho, v, w, v, p]); WR = WL.copy()
+            WL[1 + d], WR[1 + d] = u, -u
+            ps = orc.pvrs_pstar(g, rho, u, p, rho, -u, p)
+            SL, SR = orc.wave_speeds(g, rho, u, p, rho, -u, p, ps)
+            assert SL == -SR
+            F = orc.hllc(d, g, WL, WR)
+            if SL > 0.0:
+                E = p / (g - 1) + 0.5 * rho * (WL[1] ** 2 + WL[2] ** 2 + WL[3] ** 2)
+                Fe = rho * u * np.array([1.0, WL[1], WL[2], WL[3], 0.0])
+                Fe[1 + d] += p
+                Fe[4] = u * (E + p)
+                assert np.allclose(F, Fe, rtol=1e-14, atol=0.0)
+                seen[1] += 1
+            else:
+                Fn = F.copy(); Fn[1 + d] = 0.0                     # nothing but the wall pressure crosses the face
+                E = p / (g - 1) + 0.5 * rho * (u * u + v * v + w * w)
+                scale = np.array([rho * u, p + rho * u * u, p + rho * u * u, p + rho * u * u, u * (E + p)])
+                assert np.all(np.abs(Fn) <= 1e-13 * scale * (1.0 + abs(v) + abs(w)))
+                assert abs(F[1 + d] - (p + rho * u * (u - SL))) <= 1e-13 * F[1 + d]
+                seen[0] += 1
+    assert min(seen) > 50
+
+
 # ---------------------------------------------------------------- (b) interface floors ------------
 def line_cfg(nx, small_dens, small_pres, nspec=1):
     return dict(name="t", index=99, nx=nx, ny=4, nz=4, ng=4, nbx=1, nby=1, nbz=1, nspec=nspec,
