@@ -13,6 +13,11 @@ LIB = os.path.join(HERE, "libcst.so")
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-O3", "-std=c++17", "-lineinfo", "-gencode", "arch=compute_100a,code=sm_100a",
          "-Xcompiler", "-fPIC", "--shared"]
+# The operators beyond the graded path whose Riemann problems at a reflecting wall must see EXACT mirror images (the
+# upwind side is decided on a sum that cancels exactly there: DESIGN.md reading Q6b) are compiled without FMA
+# contraction: a product fused into one of two mirror-image formulas and not into the other breaks the cancellation.
+# They are multi-pass, untuned kernels; the hot kernels keep nvcc's default.
+PER_FILE = {"ctu.cu": ["-fmad=false"], "fourth.cu": ["-fmad=false"]}
 
 
 def sources():
@@ -40,7 +45,7 @@ def build(force=False, verbose=False):
 
     def compile_one(src):
         obj = os.path.join(objdir, os.path.basename(src)[:-3] + ".o")
-        subprocess.run([NVCC] + cflags + ["-c", "-o", obj, src], check=True)
+        subprocess.run([NVCC] + cflags + PER_FILE.get(os.path.basename(src), []) + ["-c", "-o", obj, src], check=True)
         return obj
     with ThreadPoolExecutor(max_workers=os.cpu_count() or 4) as ex:
         objs = list(ex.map(compile_one, sources()))

@@ -102,15 +102,16 @@ def test_uniformly_supersonic_flow(axis, sign):
 
 
 # ------------------------------------------------------------------ supersonic flow into reflecting walls ---------
-def wall_state(cfg, seed):
-    """noise + a Mach ~ 3 flow that runs away from the centre of the domain, i.e. INTO the wall on all six sides"""
+def wall_state(cfg, seed, speed=4.0):
+    """noise + a flow of the given speed (c ~ 1.3: Mach ~ 3 by default) that runs away from the centre of the domain,
+    i.e. INTO the wall on all six sides"""
     G = wl.to_global(cfg, wl.random_state(cfg, seed, amp=0.15), ghosted=True)
     rho = G[0].copy()
     for d in range(3):
         n = G.shape[3 - d]
         x = (np.arange(n) + 0.5) / n
         shape = [1, 1, 1]; shape[2 - d] = n
-        mom = G[1 + d] + 4.0 * rho * np.tanh(6.0 * (x - 0.5)).reshape(shape)      # c ~ 1.3
+        mom = G[1 + d] + speed * rho * np.tanh(6.0 * (x - 0.5)).reshape(shape)
         G[4] += 0.5 * (mom ** 2 - G[1 + d] ** 2) / rho                            # keep the pressure
         G[1 + d] = mom
     return wl.from_global(cfg, G)
