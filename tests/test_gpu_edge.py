@@ -101,52 +101,6 @@ def test_uniformly_supersonic_flow(axis, sign):
     print("supersonic", axis, sign, res)
 
 
-# ------------------------------------------------------------------ supersonic flow into reflecting walls ---------
-def wall_state(cfg, seed, speed=4.0):
-    """noise + a flow of the given speed (c ~ 1.3: Mach ~ 3 by default) that runs away from the centre of the domain,
-    i.e. INTO the wall on all six sides"""
-    G = wl.to_global(cfg, wl.random_state(cfg, seed, amp=0.15), ghosted=True)
-    rho = G[0].copy()
-    for d in range(3):
-        n = G.shape[3 - d]
-        x = (np.arange(n) + 0.5) / n
-        shape = [1, 1, 1]; shape[2 - d] = n
-        mom = G[1 + d] + speed * rho * np.tanh(6.0 * (x - 0.5)).reshape(shape)
-        G[4] += 0.5 * (mom ** 2 - G[1 + d] ** 2) / rho                            # keep the pressure
-        G[1 + d] = mom
-    return wl.from_global(cfg, G)
-
-
-def wall_ties(cfg, U):
-    """number of wall faces (x direction, low side) where the PVRS speeds give S_L > 0 > S_R for the mirror-image pair
-    of first-order states: the faces on which the side the S* test picks changes the flux by O(1)"""
-    Uo = orc.fill_ghosts(cfg, U.copy())
-    g, ng, count = cfg["gamma"], cfg["ng"], 0
-    for k in range(ng, ng + cfg["nz"]):
-        for j in range(ng, ng + cfg["ny"]):
-            W = orc.cons_to_prim(g, cfg["small_pres"], Uo[0][:, k, j, ng])
-            ps = orc.pvrs_pstar(g, W[0], -W[1], W[4], W[0], W[1], W[4])
-            SL, SR = orc.wave_speeds(g, W[0], -W[1], W[4], W[0], W[1], W[4], ps)
-            count += (SL > 0.0) and (SR < 0.0)
-    return count
-
-
-@pytest.mark.parametrize("n,nb,ns", [((32, 16, 16), (1, 1, 1), 2),     # full tiles: the fast paths
-                                     ((20, 9, 12), (1, 1, 1), 1),      # ragged tiles: the general kernels
-                                     ((16, 16, 16), (2, 1, 2), 0)])    # walls on some sides of each box only
-def test_supersonic_flow_into_reflecting_walls(n, nb, ns):
-    """The two states of a reflecting-wall face are exact mirror images (u_L = -u_R, all else equal), so the numerator of
-    S* cancels EXACTLY: S* = 0 and the left state is the upwind one (S* >= 0).  Where the flow runs into the wall faster
-    than the PVRS shock speed, S_L > 0 > S_R, both sides are "pure" and the two candidate fluxes differ by O(1): the
-    choice must be taken on the exactly cancelling sum, not on the rounding error of a fused multiply-add (hydro.cuh
-    hllc: the products are rounded separately)."""
-    cfg = small_cfg(n=n, nb=nb, nspec=ns, gamma=5 / 3, bc=(2, 2, 2))
-    U = wall_state(cfg, 77)
-    assert wall_ties(cfg, U) > 10, "the state must put S_L > 0 > S_R on wall faces"
-    res = check_one_call_set(cfg, U)
-    print("walls", n, nb, res)
-
-
 # ------------------------------------------------------------------ reciprocal / square root in ulps -------------
 def test_rcp_sqrt_sequences_within_one_ulp():
     """hydro.cuh rcp_fast / sqrt_fast (MUFU seed + Newton) against IEEE 1/x and sqrt(x) over [1e-200, 1e200]."""

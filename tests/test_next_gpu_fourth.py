@@ -8,7 +8,6 @@ import torch
 from oracle import orc
 from paper_1910_12578_b200 import Context, CstError, sdc_step_nodes, workloads as wl
 from test_oracle_pins import small_cfg
-from test_gpu_edge import wall_state, wall_ties
 
 pytestmark = pytest.mark.gpu
 TOL = 1e-12
@@ -83,25 +82,6 @@ def test_A4_matches_oracle(n, nb, ns, bc, state):
     ctx.advance_A_update(Ud, Af, Uf, dt, Aoldd, [Aoldd, Af], [0.25 * dt, 0.75 * dt])
     assert comp_err(Af.cpu().numpy(), Ao).max() <= TOL
     assert comp_err(Uf.cpu().numpy(), Uno).max() <= 10 * TOL
-    ctx.destroy()
-
-
-@pytest.mark.parametrize("n,nb,seed", [((16, 12, 10), (1, 1, 1), 77), ((12, 16, 10), (2, 1, 1), 78)])
-def test_A4_with_flow_running_into_reflecting_walls(n, nb, seed):
-    """Mirror-image states on the wall faces, S_L > 0 > S_R on many of them: the upwind side hangs on an exactly
-    cancelling sum (reading Q6b), so every operation before the Riemann solve has to treat the two mirror
-    images alike -- fourth.cu is compiled without FMA contraction for this (build.py PER_FILE)."""
-    cfg = small_cfg(n=n, nb=nb, nspec=1, gamma=5 / 3, bc=(2, 2, 2))
-    U0 = wall_state(cfg, seed, speed=2.2)
-    assert wall_ties(cfg, U0) > 5
-    U = orc.fill_ghosts(cfg, U0)
-    Ao = orc.advance_A4(cfg, U)
-    assert np.isfinite(Ao).all()
-    ctx = ctx4(cfg)
-    Ad = torch.full(wl.a_shape(cfg), float("nan"), dtype=torch.float64, device=DEV)
-    ctx.advance_A(dev(U), Ad)
-    eA = comp_err(Ad.cpu().numpy(), Ao)
-    assert eA.max() <= TOL, eA
     ctx.destroy()
 
 

@@ -115,7 +115,7 @@ def test_hllc_on_mirror_image_states_a_reflecting_wall():
     approach: S_L < 0 < S_R, the star flux with NO mass through the wall and the wall pressure p + rho u c q (Rankine-
     Hugoniot across S_L).  Approach faster than the PVRS shock speed: S_L > 0 > S_R, and the textbook's first test
     (0 <= S_L: F = F_L, Toro (10.71)) decides -- the side S* >= 0 picks at S* = 0.  The CUDA path must take the same
-    side whatever the compiler fuses (tests/test_gpu_edge.py test_supersonic_flow_into_reflecting_walls)."""
+    side whatever the compiler fuses (tests/test_next_gpu_walls.py)."""
     g = 5.0 / 3.0
     rng = np.random.default_rng(31)
     seen = [0, 0]
