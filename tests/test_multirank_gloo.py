@@ -70,3 +70,16 @@ def test_sharded_workloads_keep_the_domain_and_the_state():
         bench.fill_host_state(g, U, threads=2, brick=(tuple(pc[d] * lat[d] for d in range(3)), lat))
         ref = np.nan_to_num(full[shard.local_boxes(g, part, rank)], nan=0.0)
         assert np.array_equal(U, ref)
+
+
+def test_probe_falls_back_to_the_default_path_when_the_child_fails():
+    """bench.probe_configurations: the tunable configurations (species variants, fused CFL) are offered to the timed run
+    only if a child process has checked them on the device; a child that cannot run (here: no GPU) must leave both off
+    with a note, never raise."""
+    import torch
+    import bench
+    res = bench.probe_configurations(0)
+    assert isinstance(res["variants_ok"], bool) and isinstance(res["fused_cfl_ok"], bool) and res["note"]
+    if not torch.cuda.is_available():
+        assert res["variants_ok"] is False and res["fused_cfl_ok"] is False
+        assert "default path only" in res["note"]
