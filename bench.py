@@ -696,11 +696,11 @@ def main():
 
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device (no CPU fallback)")
-    torch.cuda.set_device(local)
-    dev = torch.device("cuda", local)
     args.safe = {"variants_ok": False, "fused_cfl_ok": False, "note": "not probed"}
     if not args.no_tune and not getattr(args, "next", False):
-        args.safe = probe_configurations(local)       # a child process per rank, before this one allocates anything
+        args.safe = probe_configurations(local)       # a child process per rank, before this one has a CUDA context
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
     if world > 1:
         dist.init_process_group("nccl", device_id=dev)
         for key in ("variants_ok", "fused_cfl_ok"):   # a configuration is used only if every rank's device passed it
